@@ -1,0 +1,44 @@
+"""The seeded input generator: determinism, order-freedom, structure (no method arithmetic in it)."""
+import numpy as np
+
+from thc_synth import make_inputs, bvv_block, normal_block, CONFIGS
+
+
+def test_deterministic_and_order_free():
+    a = make_inputs(3, 4, 6, 5, 7, seed=5)
+    b = make_inputs(3, 4, 6, 5, 7, seed=5)
+    for n in ("eps", "Xo", "Xv", "Z", "B_oo", "B_ov", "B_vv", "Y", "V"):
+        assert np.array_equal(getattr(a, n), getattr(b, n))
+    idx = np.arange(100, dtype=np.uint64)
+    full = normal_block(7, 3, idx)
+    perm = np.random.default_rng(0).permutation(100)
+    assert np.array_equal(normal_block(7, 3, idx[perm]), full[perm])
+    assert np.array_equal(bvv_block(5, 3, 4, 6, 2, 5), a.B_vv[2:5])
+    c = make_inputs(3, 4, 6, 5, 7, seed=6)
+    assert not np.array_equal(a.Xo, c.Xo)
+
+
+def test_structure_and_distributions():
+    x = make_inputs(6, 30, 40, 64, 128, seed=1)
+    assert np.array_equal(x.Z, x.Z.T) and np.array_equal(x.V, x.V.T)
+    assert np.array_equal(x.B_vv, x.B_vv.transpose(0, 2, 1))
+    assert np.array_equal(x.B_oo, x.B_oo.transpose(0, 2, 1))
+    assert np.linalg.eigvalsh(x.V).min() > -1e-12
+    assert np.all(x.eps[:6] >= -1.5) and np.all(x.eps[:6] <= -0.3)
+    assert np.all(x.eps[6:] >= 0.1) and np.all(x.eps[6:] <= 3.0)
+    assert abs(x.Xv.std() * np.sqrt(64) - 1) < 0.08
+    assert abs(x.Y.std() * np.sqrt(128) - 1) < 0.05
+    # off-diagonal of (G+G^T)/2 has std 1/sqrt(2); Z scale 0.1
+    off = x.Z[np.triu_indices(64, 1)]
+    assert abs(off.std() / (0.1 / np.sqrt(2)) - 1) < 0.08
+    # Cholesky decay exp(-L / (NL/4))
+    r = x.B_vv[39].std() / x.B_vv[0].std()
+    assert abs(r / np.exp(-39 / 10.0) - 1) < 0.15
+    g = normal_block(3, 9, np.arange(200000, dtype=np.uint64))
+    assert abs(g.mean()) < 0.01 and abs(g.std() - 1) < 0.01
+    assert abs(np.mean(g ** 4) - 3) < 0.1
+
+
+def test_configs_match_baseline():
+    assert CONFIGS[0] == dict(o=5, v=20, NL=60, NP=50, NX=100, seed=0)
+    assert CONFIGS[4] == dict(o=250, v=2250, NL=7500, NP=5000, NX=10000, seed=4)
