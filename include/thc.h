@@ -1,0 +1,138 @@
+/* thc.h -- C ABI of the B200 (sm_100a) THC-RR-CCSD projected doubles residual library.
+ *
+ * What it computes (arXiv 2111.11473, "Rank-reduced coupled-cluster III"; line numbers are PAPER.md's):
+ *
+ *   R_PQ = sum_ijab Xo[i,P] Xv[a,P] Omega_ijab Xo[j,Q] Xv[b,Q]            (Eq.6 l.82, Eq.23 l.193)
+ *
+ * with the doubles amplitudes held only as THC factors t_ij^ab = sum_PQ Xo_iP Xv_aP Z_PQ Xo_jQ Xv_bQ
+ * (Eq.23 l.193), the ERIs as Cholesky vectors B^L_pq (Eq.24 l.199, t1 = 0) and, for the T2^2 terms, as THC
+ * grid factors <ia|jb> = sum_IJ Yo_iI Yv_aI V_IJ Yo_jJ Yv_bJ (Eq.17 l.141).  Omega is the closed-shell CCSD
+ * doubles residual evaluated term by term with the paper's factorised algorithms:
+ *
+ *   term 0  sigma1  Alg.1 (l.480-530)  Eq.28       term 3  sigma6  Alg.6 (l.682-730)  Eqs.32+33 = Eq.34
+ *   term 1  sigma2  Alg.2 (l.532-567)  Eq.29       term 4  sigma7  Alg.7 (l.732-773)  Eqs.35-37 (prefactor 1/2)
+ *   term 2  sigma3  Alg.3 (l.569-606)  Eq.31       term 5  sigma9  Alg.9 (l.811-843)  Eq.41, xi from Alg.8 l.5-10
+ *
+ * and E = sum_ijab (2 t_ij^ab - t_ij^ba)(ia|jb) (l.80; Cholesky ERIs).  Readings of garbled passages: DESIGN.md.
+ *
+ * Conventions
+ *   - All arrays are FP64, row-major, last index contiguous:
+ *       Xo[o][NP]  Xv[v][NP]  Z[NP][NP] (symmetric)  B_oo[NL][o][o]  B_ov[NL][o][v]  B_vv[NL][v][v] (each
+ *       B^L symmetric)  Y[o+v][NX] (occupied rows first)  V[NX][NX] (symmetric)  eps[o+v] (occupied first)
+ *       R[NP][NP].
+ *   - "device pointer" = memory of the handle's CUDA device; "host pointer" = ordinary host memory (pinned
+ *     memory makes the copies asynchronous but is not required).
+ *   - The caller owns every input and output buffer; inputs are never modified.  The library owns only the
+ *     handle.  Scratch memory is a single workspace that the caller may provide (thc_set_workspace, e.g. a
+ *     torch allocation) or that the library allocates itself with cudaMalloc on first use.
+ *   - Device entry points enqueue work on the handle's stream (thc_set_stream; default stream 0) and return
+ *     without synchronising; outputs are valid after the stream has been synchronised.
+ *   - Every function returns THC_OK (0) or a negative thc_status; nothing throws or aborts.  The failing CUDA
+ *     error (if any) is kept in the handle: thc_last_cuda_error.
+ *   - Pointers must be 8-byte aligned; 16-byte alignment (and even o, v, NP, NX) selects the vectorised
+ *     load path, anything else the scalar one.  There is no CPU fallback of any kind.
+ */
+#ifndef THC_H_
+#define THC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct thc_handle thc_handle;
+
+typedef enum {
+  THC_OK = 0,
+  THC_ERR_INVALID_ARG = -1,   /* null pointer, non-positive size, misaligned pointer            */
+  THC_ERR_OVERFLOW = -2,      /* a buffer size does not fit in 63 bits                          */
+  THC_ERR_NO_MEMORY = -3,     /* workspace too small / cudaMalloc failed                        */
+  THC_ERR_CUDA = -4,          /* a CUDA call or kernel launch failed (see thc_last_cuda_error)  */
+  THC_ERR_NO_DEVICE = -5      /* no sm_100 device visible                                       */
+} thc_status;
+
+/* Bits of thc_options.term_mask (terms to evaluate; 0 means all). */
+enum { THC_TERM_S1 = 1, THC_TERM_S2 = 2, THC_TERM_S3 = 4, THC_TERM_S6 = 8, THC_TERM_S7 = 16, THC_TERM_S9 = 32,
+       THC_TERM_ALL = 63 };
+
+typedef struct {
+  int64_t bL;               /* Cholesky vectors per L-block of the Alg.1/2/3/8 loop (0 = auto)              */
+  int64_t bP7;              /* amplitude-grid rows per block of Alg.7 (0 = auto)                            */
+  int64_t bX;               /* amplitude-grid rows per block of Alg.6 (0 = auto; rounded up to 16)          */
+  int64_t bI;               /* ERI-grid points per chunk of Alg.6 (0 = auto)                                */
+  int64_t workspace_bytes_max; /* cap for the auto block-size choice (0 = 75 % of free device memory)       */
+  int32_t term_mask;        /* THC_TERM_* bits, 0 = all                                                     */
+  int32_t device;           /* CUDA device ordinal, -1 = current device                                     */
+} thc_options;
+
+/* Create a handle for one problem shape.  (o, v, NL, NP, NX) as in BASELINE.json / PAPER.md l.47-54
+ * (N_o, N_v, N_CD, N_aux, N_THC).  `opt` may be NULL.  Chooses block sizes, computes the workspace size. */
+int thc_setup(thc_handle** h, int64_t o, int64_t v, int64_t NL, int64_t NP, int64_t NX, const thc_options* opt);
+int thc_destroy(thc_handle* h);
+
+/* Workspace the device-pointer entry points need (bytes); thc_workspace_bytes_host: what thc_residual_host
+ * needs (the same plus staging copies of every input and of R).  A caller may provide a device buffer of at least
+ * that size (256-byte aligned; it stays owned by the caller and must outlive every call that uses the handle);
+ * otherwise the library allocates one with cudaMalloc on first use and frees it in thc_destroy. */
+int64_t thc_workspace_bytes(const thc_handle* h);
+int64_t thc_workspace_bytes_host(const thc_handle* h);
+int thc_set_workspace(thc_handle* h, void* device_ptr, int64_t bytes);
+/* CUDA stream (a cudaStream_t passed as void*) all work of this handle is enqueued on. */
+int thc_set_stream(thc_handle* h, void* cuda_stream);
+
+/* Block sizes actually in use: out[0..3] = bL, bP7, bX, bI. */
+int thc_get_blocks(const thc_handle* h, int64_t out[4]);
+
+/* R_PQ (device pointers; asynchronous).  Argument order follows the north_star:
+ * thc_residual(X^o, X^v, Z, B_ov, B_oo, B_vv, Y, V, eps) -> R_PQ.                                     */
+int thc_residual(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
+                 const double* B_oo, const double* B_vv, const double* Y, const double* V, const double* eps,
+                 double* R);
+
+/* As thc_residual, and also writes each term separately (device pointers, any of them may be NULL):
+ * terms[0..5] = sigma1, sigma2, sigma3, sigma6, sigma7, sigma9, each [NP][NP];  xi_oo[o][o] (Eq.39 l.280),
+ * xi_vv[v][v] (Eq.40 l.283).  R may be NULL.                                                            */
+int thc_residual_terms(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
+                       const double* B_oo, const double* B_vv, const double* Y, const double* V,
+                       const double* eps, double* R, double* const terms[6], double* xi_oo, double* xi_vv);
+
+/* Correlation energy E = sum_L [ 2 a^L.Z.a^L - sum_PQ Z_PQ E^L_PQ E^L_QP ] (factorised form of
+ * sum (2t - t^x)(ia|jb); a^L, E^L from Alg.8 l.5-6).  Device pointers in, one double written to the HOST
+ * address E_host; synchronises the stream.                                                             */
+int thc_energy(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
+               double* E_host);
+
+/* End-to-end entry with HOST buffers: copies every input host->device on the handle's stream, evaluates
+ * R (and E if E_host != NULL), copies R device->host into R_host[NP][NP], synchronises.  The staging
+ * buffers are part of the workspace (thc_workspace_bytes_host includes them).                       */
+int thc_residual_host(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
+                      const double* B_oo, const double* B_vv, const double* Y, const double* V,
+                      const double* eps, double* R_host, double* E_host);
+
+/* Number of kernels this handle has launched since creation (its own kernels only; no library calls). */
+int64_t thc_kernel_launches(const thc_handle* h);
+/* Algorithmic FP64 flop count of one residual evaluation for this shape (SURVEY.md 8(a) formulas). */
+double thc_algorithmic_flops(const thc_handle* h);
+
+/* Bare FP64 DMMA GEMM of the library (the kernel every GEMM chain uses), exposed for tests and roofline
+ * measurement:  C[M][N] = alpha * sum_k A(m,k) B(n,k) + beta * C,  A(m,k) = A[m*lda+k] if a_kmajor else
+ * A[k*lda+m];  B(n,k) = B[n*ldb+k] if b_kmajor else B[k*ldb+n].  Device pointers, asynchronous.        */
+int thc_dgemm(thc_handle* h, int a_kmajor, int b_kmajor, int64_t M, int64_t N, int64_t K, double alpha,
+              const double* A, int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc);
+
+/* Alg.6 line 11 (l.714) alone, for tests and roofline measurement:
+ * H[p][q][r] (+)= sum_I (E[I][p][q] F[I][p][r] + E[I][p][r] F[I][p][q]) G[I][q][r]
+ * E, F: [nI][nPp][NPp], G: [nI][NPp][NPp], H: [nPp][NPp][NPp]; NPp a multiple of 32, nPp of 16 (padded
+ * extents; padded entries are computed from whatever the padding holds and must be ignored).           */
+int thc_triple_product(thc_handle* h, int64_t nI, int64_t nPp, int64_t NPp, const double* E, const double* F,
+                       const double* G, double* H, int accumulate);
+
+const char* thc_strerror(int status);
+int thc_last_cuda_error(const thc_handle* h);   /* the cudaError_t of the last THC_ERR_CUDA, else 0 */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* THC_H_ */

@@ -1,0 +1,241 @@
+"""Thin Python binding of the C-ABI library `libthc_b200.so` (include/thc.h).
+
+Argument marshalling only: every step of the residual/energy evaluation runs in the
+library's own CUDA kernels.  torch is used for device memory and streams, nothing else.
+There is no CPU path: importing works without a GPU (the CPU test-suite checks the
+exported symbols), but every compute entry point raises if the library or a CUDA device
+is missing.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libthc_b200.so")
+SRC = os.path.join(_HERE, "csrc", "thc_lib.cu")
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+              "-shared", "-Xcompiler", "-fPIC"]
+
+# every symbol include/thc.h declares
+SYMBOLS = ("thc_setup", "thc_destroy", "thc_workspace_bytes", "thc_workspace_bytes_host", "thc_set_workspace",
+           "thc_set_stream", "thc_get_blocks", "thc_residual", "thc_residual_terms", "thc_energy",
+           "thc_residual_host", "thc_kernel_launches", "thc_algorithmic_flops", "thc_dgemm",
+           "thc_triple_product", "thc_strerror", "thc_last_cuda_error")
+
+TERM_NAMES = ("s1", "s2", "s3", "s6", "s7", "s9")
+TERM_BITS = dict(s1=1, s2=2, s3=4, s6=8, s7=16, s9=32)
+
+
+class ThcError(RuntimeError):
+    pass
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile csrc/thc_lib.cu for sm_100a into libthc_b200.so (in-tree)."""
+    deps = [os.path.join(_HERE, "csrc", f) for f in os.listdir(os.path.join(_HERE, "csrc"))]
+    deps.append(os.path.join(os.path.dirname(_HERE), "include", "thc.h"))
+    if (not force and os.path.exists(LIB_PATH)
+            and all(os.path.getmtime(LIB_PATH) >= os.path.getmtime(d) for d in deps)):
+        return LIB_PATH
+    nvcc = os.environ.get("NVCC", "nvcc")
+    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB_PATH, SRC]
+    r = subprocess.run(cmd, capture_output=True, text=True)
+    if r.returncode != 0:
+        raise ThcError("nvcc failed:\n" + r.stdout + r.stderr)
+    if verbose:
+        print(r.stderr)
+    return LIB_PATH
+
+
+class _Options(ctypes.Structure):
+    _fields_ = [("bL", ctypes.c_int64), ("bP7", ctypes.c_int64), ("bX", ctypes.c_int64), ("bI", ctypes.c_int64),
+                ("workspace_bytes_max", ctypes.c_int64), ("term_mask", ctypes.c_int32), ("device", ctypes.c_int32)]
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load the shared library (raises ThcError if it has not been built)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ThcError(f"{LIB_PATH} not found: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                       "(there is no fallback path)")
+    L = ctypes.CDLL(LIB_PATH)
+    P, D, I64, VP = ctypes.c_void_p, ctypes.c_double, ctypes.c_int64, ctypes.c_void_p
+    L.thc_setup.argtypes = [ctypes.POINTER(VP), I64, I64, I64, I64, I64, ctypes.POINTER(_Options)]
+    L.thc_destroy.argtypes = [VP]
+    L.thc_workspace_bytes.argtypes = [VP]
+    L.thc_workspace_bytes.restype = I64
+    L.thc_workspace_bytes_host.argtypes = [VP]
+    L.thc_workspace_bytes_host.restype = I64
+    L.thc_set_workspace.argtypes = [VP, P, I64]
+    L.thc_set_stream.argtypes = [VP, P]
+    L.thc_get_blocks.argtypes = [VP, ctypes.POINTER(I64 * 4)]
+    L.thc_residual.argtypes = [VP] + [P] * 10
+    L.thc_residual_terms.argtypes = [VP] + [P] * 10 + [ctypes.POINTER(P * 6), P, P]
+    L.thc_energy.argtypes = [VP, P, P, P, P, ctypes.POINTER(D)]
+    L.thc_residual_host.argtypes = [VP] + [P] * 10 + [ctypes.POINTER(D)]
+    L.thc_kernel_launches.argtypes = [VP]
+    L.thc_kernel_launches.restype = I64
+    L.thc_algorithmic_flops.argtypes = [VP]
+    L.thc_algorithmic_flops.restype = D
+    L.thc_dgemm.argtypes = [VP, ctypes.c_int, ctypes.c_int, I64, I64, I64, D, P, I64, P, I64, D, P, I64]
+    L.thc_triple_product.argtypes = [VP, I64, I64, I64, P, P, P, P, ctypes.c_int]
+    L.thc_strerror.argtypes = [ctypes.c_int]
+    L.thc_strerror.restype = ctypes.c_char_p
+    L.thc_last_cuda_error.argtypes = [VP]
+    for name in SYMBOLS:
+        getattr(L, name)          # AttributeError if a declared symbol is missing
+    _lib = L
+    return L
+
+
+def _check(st: int, h=None):
+    if st != 0:
+        msg = lib().thc_strerror(st).decode()
+        if h is not None and st == -4:
+            msg += f" [cudaError {lib().thc_last_cuda_error(h)}]"
+        raise ThcError(f"thc status {st}: {msg}")
+
+
+def _dev_ptr(t, name, numel=None):
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous():
+        raise ThcError(f"{name}: need a contiguous float64 CUDA tensor")
+    if numel is not None and t.numel() != numel:
+        raise ThcError(f"{name}: expected {numel} elements, got {t.numel()}")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _host_ptr(t, name, numel):
+    import torch
+    if not isinstance(t, torch.Tensor) or t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous():
+        raise ThcError(f"{name}: need a contiguous float64 CPU tensor")
+    if t.numel() != numel:
+        raise ThcError(f"{name}: expected {numel} elements, got {t.numel()}")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+class Thc:
+    """One problem shape (thc_setup ... thc_destroy).  Methods mirror the C entry points."""
+
+    def __init__(self, o, v, NL, NP, NX, *, bL=0, bP7=0, bX=0, bI=0, workspace_bytes_max=0, term_mask=0,
+                 device=-1, torch_workspace=True):
+        import torch
+        if not torch.cuda.is_available():
+            raise ThcError("no CUDA device: the THC residual has no CPU path")
+        self.o, self.v, self.NL, self.NP, self.NX = o, v, NL, NP, NX
+        self._h = ctypes.c_void_p()
+        opt = _Options(bL, bP7, bX, bI, workspace_bytes_max, term_mask, device)
+        _check(lib().thc_setup(ctypes.byref(self._h), o, v, NL, NP, NX, ctypes.byref(opt)))
+        self._ws = None
+        self._torch_ws = torch_workspace
+        self._device = torch.device("cuda", torch.cuda.current_device() if device < 0 else device)
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().thc_destroy(self._h)
+            self._h = ctypes.c_void_p()
+            self._ws = None
+
+    __del__ = close
+
+    # ---- plumbing -----------------------------------------------------------------------------------------
+    def _prepare(self, nbytes):
+        """Workspace from torch's allocator, work on torch's current stream."""
+        import torch
+        if self._torch_ws and (self._ws is None or self._ws.numel() < nbytes):
+            self._ws = None
+            self._ws = torch.empty(nbytes, dtype=torch.uint8, device=self._device)
+            _check(lib().thc_set_workspace(self._h, ctypes.c_void_p(self._ws.data_ptr()), self._ws.numel()), self._h)
+        _check(lib().thc_set_stream(self._h, ctypes.c_void_p(torch.cuda.current_stream(self._device).cuda_stream)))
+
+    @property
+    def workspace_bytes(self):
+        return int(lib().thc_workspace_bytes(self._h))
+
+    @property
+    def workspace_bytes_host(self):
+        return int(lib().thc_workspace_bytes_host(self._h))
+
+    @property
+    def blocks(self):
+        out = (ctypes.c_int64 * 4)()
+        _check(lib().thc_get_blocks(self._h, ctypes.byref(out)))
+        return dict(bL=out[0], bP7=out[1], bX=out[2], bI=out[3])
+
+    @property
+    def kernel_launches(self):
+        return int(lib().thc_kernel_launches(self._h))
+
+    @property
+    def algorithmic_flops(self):
+        return float(lib().thc_algorithmic_flops(self._h))
+
+    def _in_ptrs(self, Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps, conv):
+        o, v, NL, NP, NX = self.o, self.v, self.NL, self.NP, self.NX
+        return [conv(Xo, "Xo", o * NP), conv(Xv, "Xv", v * NP), conv(Z, "Z", NP * NP),
+                conv(B_ov, "B_ov", NL * o * v), conv(B_oo, "B_oo", NL * o * o), conv(B_vv, "B_vv", NL * v * v),
+                conv(Y, "Y", (o + v) * NX), conv(V, "V", NX * NX), conv(eps, "eps", o + v)]
+
+    # ---- entry points ---------------------------------------------------------------------------------------
+    def thc_residual(self, Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps, out=None):
+        """R_PQ [NP, NP] (device tensor; asynchronous on torch's current stream)."""
+        import torch
+        self._prepare(self.workspace_bytes)
+        R = out if out is not None else torch.empty(self.NP, self.NP, dtype=torch.float64, device=self._device)
+        ptrs = self._in_ptrs(Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps, _dev_ptr)
+        _check(lib().thc_residual(self._h, *ptrs, _dev_ptr(R, "R", self.NP * self.NP)), self._h)
+        return R
+
+    def thc_residual_terms(self, Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps):
+        """dict with R, s1, s2, s3, s6, s7, s9 [NP, NP], xi_oo [o, o], xi_vv [v, v] (device tensors)."""
+        import torch
+        self._prepare(self.workspace_bytes)
+        kw = dict(dtype=torch.float64, device=self._device)
+        res = {k: torch.empty(self.NP, self.NP, **kw) for k in ("R",) + TERM_NAMES}
+        res["xi_oo"] = torch.empty(self.o, self.o, **kw)
+        res["xi_vv"] = torch.empty(self.v, self.v, **kw)
+        terms = (ctypes.c_void_p * 6)(*[res[k].data_ptr() for k in TERM_NAMES])
+        ptrs = self._in_ptrs(Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps, _dev_ptr)
+        _check(lib().thc_residual_terms(self._h, *ptrs, _dev_ptr(res["R"], "R"), ctypes.byref(terms),
+                                        _dev_ptr(res["xi_oo"], "xi_oo"), _dev_ptr(res["xi_vv"], "xi_vv")), self._h)
+        return res
+
+    def thc_energy(self, Xo, Xv, Z, B_ov) -> float:
+        self._prepare(self.workspace_bytes)
+        o, v, NL, NP = self.o, self.v, self.NL, self.NP
+        E = ctypes.c_double(0.0)
+        _check(lib().thc_energy(self._h, _dev_ptr(Xo, "Xo", o * NP), _dev_ptr(Xv, "Xv", v * NP),
+                                _dev_ptr(Z, "Z", NP * NP), _dev_ptr(B_ov, "B_ov", NL * o * v), ctypes.byref(E)), self._h)
+        return E.value
+
+    def thc_residual_host(self, Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps, R_host, want_energy=True):
+        """End-to-end entry: HOST tensors in, R written into the host tensor R_host, returns E (or None)."""
+        self._prepare(self.workspace_bytes_host)
+        ptrs = self._in_ptrs(Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps, _host_ptr)
+        E = ctypes.c_double(0.0)
+        _check(lib().thc_residual_host(self._h, *ptrs, _host_ptr(R_host, "R_host", self.NP * self.NP),
+                                       ctypes.byref(E) if want_energy else None), self._h)
+        return E.value if want_energy else None
+
+    def thc_dgemm(self, a_kmajor, b_kmajor, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc):
+        # room for the split-K partial tiles of a skinny product (at most 64 splits of < 148 tiles)
+        self._prepare(self.workspace_bytes + 8 * 64 * min(M * N, 148 * 128 * 128) + 4096)
+        _check(lib().thc_dgemm(self._h, int(a_kmajor), int(b_kmajor), M, N, K, alpha, _dev_ptr(A, "A"), lda,
+                               _dev_ptr(B, "B"), ldb, beta, _dev_ptr(C, "C"), ldc), self._h)
+
+    def thc_triple_product(self, nI, nPp, NPp, E, F, G, H, accumulate):
+        self._prepare(self.workspace_bytes)
+        _check(lib().thc_triple_product(self._h, nI, nPp, NPp, _dev_ptr(E, "E", nI * nPp * NPp),
+                                        _dev_ptr(F, "F", nI * nPp * NPp), _dev_ptr(G, "G", nI * NPp * NPp),
+                                        _dev_ptr(H, "H", nPp * NPp * NPp), int(accumulate)), self._h)
+
+
+def thc_setup(o, v, NL, NP, NX, **options) -> Thc:
+    return Thc(o, v, NL, NP, NX, **options)

@@ -1,0 +1,255 @@
+// Host-side plumbing of the library: handle, bump-allocated workspace, launch helpers.
+// Every launch goes through Ctx so that (a) the same code path can be run "dry" to size the workspace,
+// (b) launches are counted (thc_kernel_launches) and (c) the first CUDA error is latched.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <algorithm>
+#include "../../include/thc.h"
+#include "thc_gemm.cuh"
+#include "thc_kernels.cuh"
+
+struct thc_handle {
+  int64_t o, v, NL, NP, NX;
+  int64_t bL, bP7, bX, bI;           // block sizes in use
+  int32_t term_mask;
+  int device, sms;
+  cudaStream_t stream;
+  void* ws;                          // workspace base (caller's or ours)
+  int64_t ws_bytes;                  // size of ws
+  bool ws_owned;
+  int64_t need_bytes;                // what the plan needs with the current block sizes
+  int64_t launches;
+  int last_cuda;
+  bool smem_configured;
+};
+
+namespace thc {
+
+// Bump allocator over the workspace.  In dry mode it only tracks the high-water mark.
+struct Arena {
+  char* base = nullptr;
+  int64_t cap = 0, top = 0, peak = 0;
+  bool dry = true, overflow = false;
+  double* alloc(i64 n_doubles) {
+    i64 bytes = (n_doubles * 8 + 255) / 256 * 256;
+    i64 at = top;
+    top += bytes;
+    peak = std::max(peak, top);
+    if (!dry && top > cap) overflow = true;
+    return reinterpret_cast<double*>(base + at);
+  }
+  i64 mark() const { return top; }
+  void release(i64 m) { top = m; }
+};
+
+struct Gemm {
+  int M, N, K;
+  const double* A; i64 lda; bool akm;
+  const double* B; i64 ldb; bool bkm;
+  double* C; i64 ldc;
+  int nbatch = 1; i64 sAb = 0, sBb = 0, sCb = 0;
+  int nkb = 1; i64 sAk = 0, sBk = 0;
+  double alpha_ = 1.0, beta_ = 0.0;
+  const double* aux_ = nullptr; i64 ldaux = 0, sAuxb = 0;
+  // A(m,k): am == 'K' -> A[m*lda + k], 'M' -> A[k*lda + m].  B(n,k): bm == 'K' -> B[n*ldb + k], 'N' -> B[k*ldb + n].
+  Gemm(const double* A_, i64 lda_, char am, const double* B_, i64 ldb_, char bm, double* C_, i64 ldc_, i64 M_, i64 N_, i64 K_)
+      : M((int)M_), N((int)N_), K((int)K_), A(A_), lda(lda_), akm(am == 'K'), B(B_), ldb(ldb_), bkm(bm == 'K'), C(C_), ldc(ldc_) {}
+  Gemm& batch(i64 n, i64 sa, i64 sb, i64 sc) { nbatch = (int)n; sAb = sa; sBb = sb; sCb = sc; return *this; }
+  Gemm& kbatch(i64 n, i64 sa, i64 sb) { nkb = (int)n; sAk = sa; sBk = sb; return *this; }
+  Gemm& ab(double a, double b) { alpha_ = a; beta_ = b; return *this; }
+  Gemm& aux(const double* p, i64 ld, i64 sb) { aux_ = p; ldaux = ld; sAuxb = sb; return *this; }
+};
+
+// tile configurations of dgemm_kernel
+#define THC_BIG 128, 128, 16, 2, 4, 4
+#define THC_SMALL 64, 64, 16, 2, 2, 4
+constexpr int BIG_THREADS = 256, SMALL_THREADS = 128;
+constexpr int gemm_smem_bytes(int BM, int BN, int BK, int ST, bool akm, bool bkm) {
+  return ST * ((akm ? BM * BK : BK * (BM + 2)) + (bkm ? BN * BK : BK * (BN + 2))) * 8;
+}
+
+template <bool AKM, bool BKM, bool AL16>
+static cudaError_t launch_gemm_variant(bool big, dim3 grid, cudaStream_t st, const GemmParams& p) {
+  if (big) {
+    auto k = dgemm_kernel<THC_BIG, AKM, BKM, AL16>;
+    int sm = gemm_smem_bytes(128, 128, 16, 4, AKM, BKM);
+    static bool done = false;
+    if (!done) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, sm); done = true; }
+    k<<<grid, BIG_THREADS, sm, st>>>(p);
+  } else {
+    auto k = dgemm_kernel<THC_SMALL, AKM, BKM, AL16>;
+    int sm = gemm_smem_bytes(64, 64, 16, 4, AKM, BKM);
+    static bool done = false;
+    if (!done) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, sm); done = true; }
+    k<<<grid, SMALL_THREADS, sm, st>>>(p);
+  }
+  return cudaPeekAtLastError();
+}
+
+struct Ctx {
+  thc_handle* h;
+  Arena ar;
+  bool dry;
+  int status = THC_OK;
+  i64 splitk_need = 0;          // doubles of split-K scratch the plan needs (dry) ...
+  double* splitk = nullptr;     // ... and the buffer (real run)
+  i64 splitk_cap = 0;
+
+  bool ok() const { return status == THC_OK; }
+  void check(cudaError_t e) {
+    if (e != cudaSuccess && status == THC_OK) { status = THC_ERR_CUDA; h->last_cuda = (int)e; }
+  }
+  void launched() { h->launches++; check(cudaPeekAtLastError()); }
+  int ew_blocks(i64 n, int per = 256) const { return (int)std::max<i64>(1, std::min<i64>((n + per - 1) / per, (i64)h->sms * 16)); }
+
+  // ---- GEMM ----------------------------------------------------------------------------------------------------
+  void gemm(const Gemm& g) {
+    if (g.M <= 0 || g.N <= 0 || g.nbatch <= 0) return;
+    const i64 tb = (i64)((g.M + 127) / 128) * ((g.N + 127) / 128) * g.nbatch;
+    const bool big = (g.M > 64 && g.N > 64 && tb * 2 >= h->sms);
+    const int BMN = big ? 128 : 64;
+    const i64 tiles_mn = (i64)((g.M + BMN - 1) / BMN) * ((g.N + BMN - 1) / BMN);
+    const i64 tiles = tiles_mn * g.nbatch;
+    const i64 kiters = (i64)g.nkb * ((g.K + 15) / 16);
+    int splits = 1;
+    if (tiles < h->sms && kiters >= 16) {
+      splits = (int)std::min<i64>(std::min<i64>((2 * h->sms + tiles - 1) / tiles, kiters / 8), 64);
+      if (splits < 1) splits = 1;
+    }
+    const i64 per = (i64)g.nbatch * g.M * g.N;
+    if (splits > 1) splitk_need = std::max(splitk_need, per * splits);
+    if (dry || !ok()) return;
+    if (splits > 1 && per * splits > splitk_cap) { status = THC_ERR_NO_MEMORY; return; }
+
+    GemmParams p;
+    p.A = g.A; p.B = g.B; p.aux = g.aux_;
+    p.M = g.M; p.N = g.N; p.K = g.K;
+    p.lda = g.lda; p.ldb = g.ldb; p.ldaux = g.ldaux;
+    p.batch = g.nbatch; p.sAb = g.sAb; p.sBb = g.sBb; p.sAuxb = g.sAuxb;
+    p.kbatch = g.nkb; p.sAk = g.sAk; p.sBk = g.sBk;
+    p.splits = splits; p.alpha = g.alpha_; p.beta = g.beta_;
+    if (splits > 1) { p.C = splitk; p.ldc = g.N; p.sCb = (i64)g.M * g.N; p.sCs = per; }
+    else            { p.C = g.C; p.ldc = g.ldc; p.sCb = g.sCb; p.sCs = 0; }
+
+    auto even = [](i64 x) { return (x & 1) == 0; };
+    const bool al16 = ((reinterpret_cast<uintptr_t>(g.A) | reinterpret_cast<uintptr_t>(g.B)) & 15) == 0 && even(g.lda) &&
+                      even(g.ldb) && even(g.sAb) && even(g.sBb) && even(g.sAk) && even(g.sBk);
+    i64 zdim = (i64)g.nbatch * splits;
+    if (zdim > 65535) { status = THC_ERR_INVALID_ARG; return; }
+    dim3 grid((unsigned)tiles_mn, 1, (unsigned)zdim);
+    cudaError_t e;
+    const int sel = (g.akm ? 4 : 0) | (g.bkm ? 2 : 0) | (al16 ? 1 : 0);
+    switch (sel) {
+      case 7: e = launch_gemm_variant<true, true, true>(big, grid, h->stream, p); break;
+      case 6: e = launch_gemm_variant<true, true, false>(big, grid, h->stream, p); break;
+      case 5: e = launch_gemm_variant<true, false, true>(big, grid, h->stream, p); break;
+      case 4: e = launch_gemm_variant<true, false, false>(big, grid, h->stream, p); break;
+      case 3: e = launch_gemm_variant<false, true, true>(big, grid, h->stream, p); break;
+      case 2: e = launch_gemm_variant<false, true, false>(big, grid, h->stream, p); break;
+      case 1: e = launch_gemm_variant<false, false, true>(big, grid, h->stream, p); break;
+      default: e = launch_gemm_variant<false, false, false>(big, grid, h->stream, p); break;
+    }
+    h->launches++;
+    check(e);
+    if (splits > 1) {
+      ReduceParams r;
+      r.part = splitk; r.dst = g.C; r.aux = g.aux_;
+      r.M = g.M; r.N = g.N; r.batch = g.nbatch; r.splits = splits;
+      r.ldd = g.ldc; r.sDb = g.sCb; r.ldaux = g.ldaux; r.sAuxb = g.sAuxb;
+      r.alpha = g.alpha_; r.beta = g.beta_;
+      reduce_splits_kernel<<<ew_blocks(per), 256, 0, h->stream>>>(r);
+      launched();
+    }
+  }
+
+  // ---- element-wise / reduction launches -------------------------------------------------------------------------
+#define THC_EW(kernel, n, ...)                                          \
+  do {                                                                  \
+    if (dry || !ok()) return;                                           \
+    kernel<<<ew_blocks(n), 256, 0, h->stream>>>(__VA_ARGS__);           \
+    launched();                                                         \
+  } while (0)
+
+  void transpose(const double* in, double* out, i64 rows, i64 cols) {
+    if (dry || !ok()) return;
+    dim3 grid((unsigned)((cols + 31) / 32), (unsigned)((rows + 31) / 32)), blk(32, 8);
+    transpose_kernel<<<grid, blk, 0, h->stream>>>(in, out, (int)rows, (int)cols);
+    launched();
+  }
+  void fill(double* x, i64 n, double val) { THC_EW(fill_kernel, n, x, n, val); }
+  void hadamard(const double* a, const double* b, double* out, i64 n) { THC_EW(hadamard_kernel, n, a, b, out, n); }
+  void axpby(const double* a, const double* b, double ca, double cb, double* out, i64 n) {
+    THC_EW(axpby_kernel, n, a, b, ca, cb, out, n);
+  }
+  void had2_diff(const double* a, const double* b, const double* c, const double* d, double* out, i64 n) {
+    THC_EW(had2_diff_kernel, n, a, b, c, d, out, n);
+  }
+  void combine(double* Mo, const double* Mv, const double* omat, const double* vmat, double* C3, i64 np2, i64 nl) {
+    THC_EW(combine_kernel, np2, Mo, Mv, omat, vmat, C3, np2, (int)nl);
+  }
+  void rowdot(const double* X, i64 ldx, const double* T, i64 sTb, i64 ldT, double* out, i64 ldo, i64 nb, i64 nr, i64 n) {
+    THC_EW(rowdot_kernel, nb * nr, X, ldx, T, sTb, ldT, out, ldo, (int)nb, (int)nr, (int)n);
+  }
+  void coldot(const double* X, i64 ldx, const double* T, i64 sTb, i64 ldT, double* out, i64 ldo, i64 nb, i64 nc, i64 n) {
+    THC_EW(coldot_kernel, nb * nc, X, ldx, T, sTb, ldT, out, ldo, (int)nb, (int)nc, (int)n);
+  }
+  void rowscale(const double* X, i64 ldx, const double* Mrow, i64 ldm, const double* add, double alpha, double* out,
+                i64 nb, i64 n, i64 nc) {
+    THC_EW(rowscale_kernel, nb * n * nc, X, ldx, Mrow, ldm, add, alpha, out, (int)nb, (int)n, (int)nc);
+  }
+  void rowscale_inplace(double* T, const double* Mrow, i64 ldm, double alpha, i64 nb, i64 n, i64 nc) {
+    THC_EW(rowscale_inplace_kernel, nb * n * nc, T, Mrow, ldm, alpha, (int)nb, (int)n, (int)nc);
+  }
+  void qm(double* G1, const double* Xo, const double* ZA, i64 o, i64 nl, i64 NP) {
+    THC_EW(qm_kernel, o * nl * NP, G1, Xo, ZA, (int)o, (int)nl, (int)NP);
+  }
+  void symmetrize(const double* P, double* out, i64 n, double scale) {
+    if (dry || !ok()) return;
+    dim3 grid((unsigned)((n + 31) / 32), (unsigned)((n + 31) / 32)), blk(32, 8);
+    symmetrize_kernel<<<grid, blk, 0, h->stream>>>(P, out, (int)n, scale);
+    launched();
+  }
+  void fock(const double* eps, const double* xi_oo, const double* xi_vv, double* FooT, double* Fvv, i64 o, i64 v) {
+    THC_EW(fock_kernel, o * o + v * v, eps, xi_oo, xi_vv, FooT, Fvv, (int)o, (int)v);
+  }
+  void sum6(const double* const t[6], double* out, i64 n) {
+    THC_EW(sum6_kernel, n, t[0], t[1], t[2], t[3], t[4], t[5], out, n);
+  }
+  // partial sums for the energy; `partial` must hold dot_blocks() / zee_blocks() doubles
+  int dot_blocks(i64 n) const { return ew_blocks(n, 1024); }
+  void dot_partial(const double* a, const double* b, i64 n, double* partial) {
+    if (dry || !ok()) return;
+    dot_partial_kernel<<<dot_blocks(n), 256, 0, h->stream>>>(a, b, n, partial);
+    launched();
+  }
+  i64 zee_blocks(i64 NP, i64 nl) const { i64 t = (NP + 31) / 32; return t * t * nl; }
+  void zee_partial(const double* Z, const double* E, i64 NP, i64 nl, double* partial) {
+    if (dry || !ok()) return;
+    unsigned t = (unsigned)((NP + 31) / 32);
+    dim3 grid(t, t, (unsigned)nl), blk(32, 8);
+    zee_partial_kernel<<<grid, blk, 0, h->stream>>>(Z, E, (int)NP, partial);
+    launched();
+  }
+  void final_sum(const double* pa, i64 na, double ca, const double* pb, i64 nb, double cb, double* out, int accumulate) {
+    if (dry || !ok()) return;
+    final_sum_kernel<<<1, 1024, 0, h->stream>>>(pa, na, ca, pb, nb, cb, out, accumulate);
+    launched();
+  }
+  void triple_product(const double* E, const double* F, const double* G, double* H, i64 nI, i64 nPp, i64 NPp, int accumulate) {
+    if (dry || !ok()) return;
+    if (!h->smem_configured) {
+      check(cudaFuncSetAttribute(triple_product_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TP_SMEM_BYTES));
+      h->smem_configured = true;
+    }
+    TripleParams p;
+    p.E = E; p.F = F; p.G = G; p.H = H;
+    p.nI = (int)nI; p.nPp = (int)nPp; p.NPp = (int)NPp; p.accumulate = accumulate;
+    i64 nrb = NPp / TP_RT;
+    dim3 grid((unsigned)(nrb * (nrb + 1)), (unsigned)(nPp / TP_PT));
+    triple_product_kernel<<<grid, 256, TP_SMEM_BYTES, h->stream>>>(p);
+    launched();
+  }
+};
+
+}  // namespace thc

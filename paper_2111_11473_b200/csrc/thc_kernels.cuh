@@ -1,0 +1,427 @@
+// Hadamard / reduction kernels (HBM-streaming) and the Alg.6 line-11 triple-product kernel (FP64 FMA pipe).
+// Citations are PAPER.md line numbers.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "thc_gemm.cuh"
+
+namespace thc {
+
+typedef long long i64;
+
+#define THC_GRID_STRIDE(idx, total) \
+  for (i64 idx = (i64)blockIdx.x * blockDim.x + threadIdx.x; idx < (total); idx += (i64)gridDim.x * blockDim.x)
+
+// out[c][r] = in[r][c]   (small factor matrices only)
+__global__ void transpose_kernel(const double* __restrict__ in, double* __restrict__ out, int rows, int cols) {
+  __shared__ double tile[32][33];
+  int c0 = blockIdx.x * 32, r0 = blockIdx.y * 32;
+  for (int j = threadIdx.y; j < 32; j += blockDim.y) {
+    int r = r0 + j, c = c0 + threadIdx.x;
+    if (r < rows && c < cols) tile[j][threadIdx.x] = in[(i64)r * cols + c];
+  }
+  __syncthreads();
+  for (int j = threadIdx.y; j < 32; j += blockDim.y) {
+    int c = c0 + j, r = r0 + threadIdx.x;
+    if (r < rows && c < cols) out[(i64)c * rows + r] = tile[threadIdx.x][j];
+  }
+}
+
+__global__ void fill_kernel(double* __restrict__ x, i64 n, double val) {
+  THC_GRID_STRIDE(i, n) x[i] = val;
+}
+
+// out = a .* b                                   (w = o .* v, Alg.3 l.596, Alg.7 l.736, Alg.9 l.817)
+__global__ void hadamard_kernel(const double* __restrict__ a, const double* __restrict__ b, double* __restrict__ out, i64 n) {
+  THC_GRID_STRIDE(i, n) out[i] = a[i] * b[i];
+}
+
+// out = ca * a + cb * b
+__global__ void axpby_kernel(const double* __restrict__ a, const double* __restrict__ b, double ca, double cb,
+                             double* __restrict__ out, i64 n) {
+  THC_GRID_STRIDE(i, n) out[i] = ca * a[i] + cb * b[i];
+}
+
+// out = a .* b - c .* d                          (E = o .* v~ - o~ .* v, Alg.9 line 9 l.835)
+__global__ void had2_diff_kernel(const double* __restrict__ a, const double* __restrict__ b, const double* __restrict__ c,
+                                 const double* __restrict__ d, double* __restrict__ out, i64 n) {
+  THC_GRID_STRIDE(i, n) out[i] = a[i] * b[i] - c[i] * d[i];
+}
+
+// Alg.1 lines 8, 12, 13 (l.502-518) and Alg.3 line 7 (l.587), for nl Cholesky vectors at once:
+//   C^l = v .* Mo^l - o .* Mv^l   (written over Mo),   C3 += sum_l Mo^l .* Mv^l
+__global__ void combine_kernel(double* __restrict__ Mo, const double* __restrict__ Mv, const double* __restrict__ omat,
+                               const double* __restrict__ vmat, double* __restrict__ C3, i64 np2, int nl) {
+  THC_GRID_STRIDE(i, np2) {
+    double ov = omat[i], vv = vmat[i], c3 = 0.0;
+    for (int l = 0; l < nl; l++) {
+      double mo = Mo[(i64)l * np2 + i], mv = Mv[(i64)l * np2 + i];
+      c3 = fma(mo, mv, c3);
+      Mo[(i64)l * np2 + i] = vv * mo - ov * mv;
+    }
+    C3[i] += c3;
+  }
+}
+
+// out[b*ldo + r] = sum_{i<n} X[r*ldx + i] * T[b*sTb + r*ldT + i]      (a^L_P: Alg.2 l.541, Alg.8 l.788; C7: Alg.7 line 9 l.749)
+__global__ void rowdot_kernel(const double* __restrict__ X, i64 ldx, const double* __restrict__ T, i64 sTb, i64 ldT,
+                              double* __restrict__ out, i64 ldo, int nb, int nr, int n) {
+  i64 total = (i64)nb * nr;
+  THC_GRID_STRIDE(idx, total) {
+    int r = (int)(idx % nr), b = (int)(idx / nr);
+    const double* x = X + (i64)r * ldx;
+    const double* tt = T + (i64)b * sTb + (i64)r * ldT;
+    double s = 0.0;
+    for (int i = 0; i < n; i++) s = fma(x[i], tt[i], s);
+    out[(i64)b * ldo + r] = s;
+  }
+}
+
+// out[b*ldo + c] = sum_{i<n} X[i*ldx + c] * T[b*sTb + i*ldT + c]      (d^L_P: Alg.2 l.549,557; sigma6 row: Alg.6 line 15 l.724)
+__global__ void coldot_kernel(const double* __restrict__ X, i64 ldx, const double* __restrict__ T, i64 sTb, i64 ldT,
+                              double* __restrict__ out, i64 ldo, int nb, int nc, int n) {
+  i64 total = (i64)nb * nc;
+  THC_GRID_STRIDE(idx, total) {
+    int c = (int)(idx % nc), b = (int)(idx / nc);
+    const double* tt = T + (i64)b * sTb + c;
+    double s = 0.0;
+    for (int i = 0; i < n; i++) s = fma(X[(i64)i * ldx + c], tt[(i64)i * ldT], s);
+    out[(i64)b * ldo + c] = s;
+  }
+}
+
+// out[(b,i)][c] = alpha * X[i][c] * Mrow[b][c] (+ add[(b,i)][c])       b < nb, i < n, c < nc
+// (Xo .* v_P, Alg.7 line 6 l.743 in scaled-factor form; 2 Xo .* K_P, Alg.7 line 4 l.739; Z_Q .* Xo, Alg.6 line 1 l.683;
+//  V_I .* Yo, Alg.6 line 2 l.686)
+__global__ void rowscale_kernel(const double* __restrict__ X, i64 ldx, const double* __restrict__ Mrow, i64 ldm,
+                                const double* __restrict__ add, double alpha, double* __restrict__ out, int nb, int n, int nc) {
+  i64 total = (i64)nb * n * nc;
+  THC_GRID_STRIDE(idx, total) {
+    int c = (int)(idx % nc);
+    i64 r = idx / nc;
+    int i = (int)(r % n), b = (int)(r / n);
+    double val = alpha * X[(i64)i * ldx + c] * Mrow[(i64)b * ldm + c];
+    if (add) val += add[idx];
+    out[idx] = val;
+  }
+}
+
+// T[(b,i)][c] = alpha * T[(b,i)][c] * Mrow[b][c]   in place            (-(SZ) .* o_P, Alg.7 line 6/7 l.743-745)
+__global__ void rowscale_inplace_kernel(double* __restrict__ T, const double* __restrict__ Mrow, i64 ldm, double alpha,
+                                        int nb, int n, int nc) {
+  i64 total = (i64)nb * n * nc;
+  THC_GRID_STRIDE(idx, total) {
+    int c = (int)(idx % nc);
+    int b = (int)((idx / nc) / n);
+    T[idx] = alpha * T[idx] * Mrow[(i64)b * ldm + c];
+  }
+}
+
+// Qm[i][(l,P)] = 2 Xo[i][P] * ZA[l][P] - G1[i][(l,P)]   in place on G1   (Alg.8 line 7 l.792 folded into line 8)
+__global__ void qm_kernel(double* __restrict__ G1, const double* __restrict__ Xo, const double* __restrict__ ZA, int o, int nl, int NP) {
+  i64 total = (i64)o * nl * NP;
+  THC_GRID_STRIDE(idx, total) {
+    int P = (int)(idx % NP);
+    i64 r = idx / NP;
+    int l = (int)(r % nl), i = (int)(r / nl);
+    G1[idx] = 2.0 * Xo[(i64)i * NP + P] * ZA[(i64)l * NP + P] - G1[idx];
+  }
+}
+
+// out = scale * (P + P^T)                        (Alg.3 line 12 l.601; Alg.9 line 10 l.839)
+__global__ void symmetrize_kernel(const double* __restrict__ Pm, double* __restrict__ out, int n, double scale) {
+  __shared__ double tile[32][33];
+  int bx = blockIdx.x, by = blockIdx.y;
+  for (int j = threadIdx.y; j < 32; j += blockDim.y) {
+    int r = bx * 32 + j, c = by * 32 + threadIdx.x;   // element of the transposed tile
+    if (r < n && c < n) tile[j][threadIdx.x] = Pm[(i64)r * n + c];
+  }
+  __syncthreads();
+  for (int j = threadIdx.y; j < 32; j += blockDim.y) {
+    int r = by * 32 + j, c = bx * 32 + threadIdx.x;
+    if (r < n && c < n) out[(i64)r * n + c] = scale * (Pm[(i64)r * n + c] + tile[threadIdx.x][j]);
+  }
+}
+
+// FooT[i][j] = delta_ij eps[i] + xi_oo[j][i];  Fvv[a][b] = delta_ab eps[o+a] + xi_vv[a][b]   (Alg.9 lines 5-6 l.823-827)
+__global__ void fock_kernel(const double* __restrict__ eps, const double* __restrict__ xi_oo, const double* __restrict__ xi_vv,
+                            double* __restrict__ FooT, double* __restrict__ Fvv, int o, int v) {
+  i64 total = (i64)o * o + (i64)v * v;
+  THC_GRID_STRIDE(idx, total) {
+    if (idx < (i64)o * o) {
+      int i = (int)(idx / o), j = (int)(idx % o);
+      FooT[idx] = xi_oo[(i64)j * o + i] + (i == j ? eps[i] : 0.0);
+    } else {
+      i64 k = idx - (i64)o * o;
+      int a = (int)(k / v), b = (int)(k % v);
+      Fvv[k] = xi_vv[k] + (a == b ? eps[o + a] : 0.0);
+    }
+  }
+}
+
+// R = sum of up to six terms
+__global__ void sum6_kernel(const double* a, const double* b, const double* c, const double* d, const double* e,
+                            const double* f, double* __restrict__ out, i64 n) {
+  THC_GRID_STRIDE(i, n) {
+    double s = 0.0;
+    if (a) s += a[i];
+    if (b) s += b[i];
+    if (c) s += c[i];
+    if (d) s += d[i];
+    if (e) s += e[i];
+    if (f) s += f[i];
+    out[i] = s;
+  }
+}
+
+// ---- energy reductions (H12): block partial sums in double-double-free pairwise form, final sum on one block.
+__device__ __forceinline__ double block_sum(double v) {
+  __shared__ double sh[32];
+  for (int off = 16; off > 0; off >>= 1) v += __shfl_down_sync(0xffffffffu, v, off);
+  int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+  __syncthreads();
+  if (l == 0) sh[w] = v;
+  __syncthreads();
+  int nw = (blockDim.x + 31) >> 5;
+  v = (threadIdx.x < nw) ? sh[threadIdx.x] : 0.0;
+  if (w == 0)
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_down_sync(0xffffffffu, v, off);
+  return v;   // valid on thread 0
+}
+
+// partial[blockIdx.x] = sum_i a[i] * b[i] over this block's grid-stride share
+__global__ void dot_partial_kernel(const double* __restrict__ a, const double* __restrict__ b, i64 n, double* __restrict__ partial) {
+  double s = 0.0;
+  THC_GRID_STRIDE(i, n) s = fma(a[i], b[i], s);
+  s = block_sum(s);
+  if (threadIdx.x == 0) partial[blockIdx.x] = s;
+}
+
+// partial[block] = sum over a 32x32 tile pair of Z[P][Q] * E[l][P][Q] * E[l][Q][P]; grid = (tiles, tiles, nl), block (32, 8)
+__global__ void zee_partial_kernel(const double* __restrict__ Z, const double* __restrict__ E, int NP, double* __restrict__ partial) {
+  __shared__ double tile[32][33];
+  const double* El = E + (i64)blockIdx.z * NP * NP;
+  int bx = blockIdx.x, by = blockIdx.y;
+  for (int j = threadIdx.y; j < 32; j += blockDim.y) {
+    int r = bx * 32 + j, c = by * 32 + threadIdx.x;
+    tile[j][threadIdx.x] = (r < NP && c < NP) ? El[(i64)r * NP + c] : 0.0;
+  }
+  __syncthreads();
+  double s = 0.0;
+  for (int j = threadIdx.y; j < 32; j += blockDim.y) {
+    int r = by * 32 + j, c = bx * 32 + threadIdx.x;
+    if (r < NP && c < NP) s = fma(Z[(i64)r * NP + c] * El[(i64)r * NP + c], tile[threadIdx.x][j], s);
+  }
+  // block reduction over 256 threads (blockDim = 32 x 8)
+  __shared__ double sh[8];
+  for (int off = 16; off > 0; off >>= 1) s += __shfl_down_sync(0xffffffffu, s, off);
+  if (threadIdx.x == 0) sh[threadIdx.y] = s;
+  __syncthreads();
+  if (threadIdx.x == 0 && threadIdx.y == 0) {
+    double tot = 0.0;
+    for (int k = 0; k < (int)blockDim.y; k++) tot += sh[k];
+    partial[((i64)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x] = tot;
+  }
+}
+
+// out[0] = ca * sum(pa[0..na)) + cb * sum(pb[0..nb))     (one block; Kahan-compensated per thread, then tree)
+__global__ void final_sum_kernel(const double* __restrict__ pa, i64 na, double ca, const double* __restrict__ pb, i64 nb,
+                                 double cb, double* __restrict__ out, int accumulate) {
+  double s = 0.0, comp = 0.0;
+  for (i64 i = threadIdx.x; i < na + nb; i += blockDim.x) {
+    double x = (i < na) ? ca * pa[i] : cb * pb[i - na];
+    double y = x - comp, tt = s + y;
+    comp = (tt - s) - y;
+    s = tt;
+  }
+  s = block_sum(s);
+  if (threadIdx.x == 0) out[0] = accumulate ? out[0] + s : s;
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// Alg.6 line 11 (l.714):  H[p][q][r] += sum_I (E_I[p][q] F_I[p][r] + E_I[p][r] F_I[p][q]) G_I[q][r]
+//
+// The bracket s_I[p](q,r) is symmetric in (q,r), so a CTA that owns the (p, q-tile, r-tile) block with the q-tile
+// strictly below the r-tile also owns the mirrored block (p, r-tile, q-tile): s is formed once (2 FP64 instr) and
+// used twice (2 FMA) -> 2 instead of 3 FP64 instructions per (p,q,r,I).  CTAs whose q-tile lies inside their r-tile
+// (the diagonal) do the plain 3-instruction update for every (q,r) of the block.
+//
+// CTA = 256 threads = 8 warps as (2 p) x (2 q) x (2 r); lane = (lp 2) x (lq 4) x (lr 4); thread tile (4 p, 2 q, 4 r)
+// => warp tile 8 x 8 x 16, CTA tile 16 x 16 x 32, 64 accumulators per thread.  Per I the CTA reads six operand
+// tiles from shared memory (E,F over (p,q); E,F over (p,r); G over (q,r); G over (r,q)), staged by cp.async in
+// chunks of TP_IC grid points, TP_STAGES deep.  Row pitches (18 / 34 doubles) make every 16-byte fragment load
+// conflict-free: see DESIGN.md section 6.
+constexpr int TP_PT = 16, TP_QT = 16, TP_RT = 32, TP_IC = 2, TP_STAGES = 3;
+constexpr int TP_PQ_PITCH = 18, TP_PR_PITCH = 34;
+constexpr int TP_OFF_EPQ = 0;
+constexpr int TP_OFF_FPQ = TP_OFF_EPQ + TP_PT * TP_PQ_PITCH;
+constexpr int TP_OFF_EPR = TP_OFF_FPQ + TP_PT * TP_PQ_PITCH;
+constexpr int TP_OFF_FPR = TP_OFF_EPR + TP_PT * TP_PR_PITCH;
+constexpr int TP_OFF_GQR = TP_OFF_FPR + TP_PT * TP_PR_PITCH;
+constexpr int TP_OFF_GRQ = TP_OFF_GQR + TP_QT * TP_PR_PITCH;
+constexpr int TP_PER_I = TP_OFF_GRQ + TP_RT * TP_PQ_PITCH;       // doubles per grid point
+constexpr int TP_STAGE = TP_PER_I * TP_IC;
+constexpr int TP_SMEM_BYTES = TP_STAGE * TP_STAGES * 8;
+
+struct TripleParams {
+  const double* E; const double* F; const double* G; double* H;
+  int nI, nPp, NPp;        // padded extents: nPp % 16 == 0, NPp % 32 == 0
+  int accumulate;
+};
+
+__device__ __forceinline__ void tp_copy_rows(double* s, int pitch, const double* g, i64 ld, int rows, int cols, int tid) {
+  // rows x cols doubles (cols % 2 == 0), 16-byte chunks
+  int cpr = cols / 2, total = rows * cpr;
+  for (int c = tid; c < total; c += 256) {
+    int r = c / cpr, cc = c % cpr;
+    cp_async16(s + r * pitch + cc * 2, g + (i64)r * ld + cc * 2, 16);
+  }
+}
+
+__global__ void __launch_bounds__(256) triple_product_kernel(const TripleParams p) {
+  extern __shared__ __align__(16) double smem[];
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int wp = warp >> 2, wq = (warp >> 1) & 1, wr = warp & 1;
+  const int lp = lane >> 4, lq = (lane >> 2) & 3, lr = lane & 3;
+  // tile coordinates: blockIdx.x enumerates (qb, rb) with qb/2 <= rb; blockIdx.y = p tile
+  const int nrb = p.NPp / TP_RT;
+  int rb = 0, qb = 0;
+  {
+    // pairs are ordered rb-major: rb = 0 has qb in [0, 2), rb = 1 has [0, 4), ...  -> offset(rb) = rb (rb + 1)
+    int x = blockIdx.x;
+    rb = (int)((sqrtf(4.0f * x + 1.0f) - 1.0f) * 0.5f);
+    while (rb * (rb + 1) > x) rb--;
+    while ((rb + 1) * (rb + 2) <= x) rb++;
+    qb = x - rb * (rb + 1);
+  }
+  (void)nrb;
+  const bool diag = (qb >> 1) == rb;
+  const int p0 = blockIdx.y * TP_PT, q0 = qb * TP_QT, r0 = rb * TP_RT;
+  const i64 ldE = p.NPp, sEI = (i64)p.nPp * p.NPp;      // E[I][p][q]
+  const i64 ldG = p.NPp, sGI = (i64)p.NPp * p.NPp;      // G[I][q][r]
+
+  // thread's indices inside the CTA tile
+  const int tp0 = wp * 8 + lp * 4;                      // 4 consecutive p
+  const int tq0 = wq * 8 + lq * 2;                      // 2 consecutive q
+  const int trA = wr * 16 + lr * 2, trB = trA + 8;      // r pairs {trA, trA+1}, {trB, trB+1}
+
+  double hqr[4][2][4], hrq[4][2][4];
+#pragma unroll
+  for (int a = 0; a < 4; a++)
+#pragma unroll
+    for (int b = 0; b < 2; b++)
+#pragma unroll
+      for (int c = 0; c < 4; c++) hqr[a][b][c] = hrq[a][b][c] = 0.0;
+
+  const int nchunks = (p.nI + TP_IC - 1) / TP_IC;
+  auto issue = [&](int ch) {
+    if (ch < nchunks) {
+      double* st = smem + (ch % TP_STAGES) * TP_STAGE;
+      for (int ii = 0; ii < TP_IC; ii++) {
+        int I = ch * TP_IC + ii;
+        if (I >= p.nI) break;
+        double* s = st + ii * TP_PER_I;
+        const double* Eg = p.E + (i64)I * sEI + (i64)p0 * ldE;
+        const double* Fg = p.F + (i64)I * sEI + (i64)p0 * ldE;
+        const double* Gg = p.G + (i64)I * sGI;
+        tp_copy_rows(s + TP_OFF_EPQ, TP_PQ_PITCH, Eg + q0, ldE, TP_PT, TP_QT, tid);
+        tp_copy_rows(s + TP_OFF_FPQ, TP_PQ_PITCH, Fg + q0, ldE, TP_PT, TP_QT, tid);
+        tp_copy_rows(s + TP_OFF_EPR, TP_PR_PITCH, Eg + r0, ldE, TP_PT, TP_RT, tid);
+        tp_copy_rows(s + TP_OFF_FPR, TP_PR_PITCH, Fg + r0, ldE, TP_PT, TP_RT, tid);
+        tp_copy_rows(s + TP_OFF_GQR, TP_PR_PITCH, Gg + (i64)q0 * ldG + r0, ldG, TP_QT, TP_RT, tid);
+        if (!diag) tp_copy_rows(s + TP_OFF_GRQ, TP_PQ_PITCH, Gg + (i64)r0 * ldG + q0, ldG, TP_RT, TP_QT, tid);
+      }
+    }
+    cp_async_commit();
+  };
+#pragma unroll
+  for (int s = 0; s < TP_STAGES - 1; s++) issue(s);
+
+  for (int ch = 0; ch < nchunks; ch++) {
+    cp_async_wait<TP_STAGES - 2>();
+    __syncthreads();
+    issue(ch + TP_STAGES - 1);
+    const double* st = smem + (ch % TP_STAGES) * TP_STAGE;
+    const int ni = min(TP_IC, p.nI - ch * TP_IC);
+    for (int ii = 0; ii < ni; ii++) {
+      const double* s = st + ii * TP_PER_I;
+      double epq[4][2], fpq[4][2], epr[4][4], fpr[4][4], gqr[2][4];
+#pragma unroll
+      for (int a = 0; a < 4; a++) {
+        double2 x = *reinterpret_cast<const double2*>(s + TP_OFF_EPQ + (tp0 + a) * TP_PQ_PITCH + tq0);
+        double2 y = *reinterpret_cast<const double2*>(s + TP_OFF_FPQ + (tp0 + a) * TP_PQ_PITCH + tq0);
+        epq[a][0] = x.x; epq[a][1] = x.y; fpq[a][0] = y.x; fpq[a][1] = y.y;
+        double2 e0 = *reinterpret_cast<const double2*>(s + TP_OFF_EPR + (tp0 + a) * TP_PR_PITCH + trA);
+        double2 e1 = *reinterpret_cast<const double2*>(s + TP_OFF_EPR + (tp0 + a) * TP_PR_PITCH + trB);
+        double2 f0 = *reinterpret_cast<const double2*>(s + TP_OFF_FPR + (tp0 + a) * TP_PR_PITCH + trA);
+        double2 f1 = *reinterpret_cast<const double2*>(s + TP_OFF_FPR + (tp0 + a) * TP_PR_PITCH + trB);
+        epr[a][0] = e0.x; epr[a][1] = e0.y; epr[a][2] = e1.x; epr[a][3] = e1.y;
+        fpr[a][0] = f0.x; fpr[a][1] = f0.y; fpr[a][2] = f1.x; fpr[a][3] = f1.y;
+      }
+#pragma unroll
+      for (int b = 0; b < 2; b++) {
+        double2 g0 = *reinterpret_cast<const double2*>(s + TP_OFF_GQR + (tq0 + b) * TP_PR_PITCH + trA);
+        double2 g1 = *reinterpret_cast<const double2*>(s + TP_OFF_GQR + (tq0 + b) * TP_PR_PITCH + trB);
+        gqr[b][0] = g0.x; gqr[b][1] = g0.y; gqr[b][2] = g1.x; gqr[b][3] = g1.y;
+      }
+      if (!diag) {
+        double grq[4][2];
+#pragma unroll
+        for (int c = 0; c < 4; c++) {
+          int r = (c < 2) ? trA + c : trB + (c - 2);
+          double2 gg = *reinterpret_cast<const double2*>(s + TP_OFF_GRQ + r * TP_PQ_PITCH + tq0);
+          grq[c][0] = gg.x; grq[c][1] = gg.y;
+        }
+#pragma unroll
+        for (int a = 0; a < 4; a++)
+#pragma unroll
+          for (int b = 0; b < 2; b++)
+#pragma unroll
+            for (int c = 0; c < 4; c++) {
+              double sv = fma(epr[a][c], fpq[a][b], epq[a][b] * fpr[a][c]);
+              hqr[a][b][c] = fma(sv, gqr[b][c], hqr[a][b][c]);
+              hrq[a][b][c] = fma(sv, grq[c][b], hrq[a][b][c]);
+            }
+      } else {
+#pragma unroll
+        for (int a = 0; a < 4; a++)
+#pragma unroll
+          for (int b = 0; b < 2; b++)
+#pragma unroll
+            for (int c = 0; c < 4; c++) {
+              double sv = fma(epr[a][c], fpq[a][b], epq[a][b] * fpr[a][c]);
+              hqr[a][b][c] = fma(sv, gqr[b][c], hqr[a][b][c]);
+            }
+      }
+    }
+  }
+  cp_async_wait<0>();
+
+  // write back: H[p][q][r]
+  const i64 sHp = (i64)p.NPp * p.NPp;
+#pragma unroll
+  for (int a = 0; a < 4; a++) {
+    double* Hp = p.H + (i64)(p0 + tp0 + a) * sHp;
+#pragma unroll
+    for (int b = 0; b < 2; b++) {
+      double* row = Hp + (i64)(q0 + tq0 + b) * p.NPp + r0;
+      double2* d0 = reinterpret_cast<double2*>(row + trA);
+      double2* d1 = reinterpret_cast<double2*>(row + trB);
+      double2 v0 = make_double2(hqr[a][b][0], hqr[a][b][1]), v1 = make_double2(hqr[a][b][2], hqr[a][b][3]);
+      if (p.accumulate) { double2 o0 = *d0, o1 = *d1; v0.x += o0.x; v0.y += o0.y; v1.x += o1.x; v1.y += o1.y; }
+      *d0 = v0; *d1 = v1;
+    }
+    if (!diag) {
+#pragma unroll
+      for (int c = 0; c < 4; c++) {
+        int r = (c < 2) ? trA + c : trB + (c - 2);
+        double2* d = reinterpret_cast<double2*>(Hp + (i64)(r0 + r) * p.NPp + q0 + tq0);
+        double2 vv = make_double2(hrq[a][0][c], hrq[a][1][c]);
+        if (p.accumulate) { double2 o = *d; vv.x += o.x; vv.y += o.y; }
+        *d = vv;
+      }
+    }
+  }
+}
+
+}  // namespace thc

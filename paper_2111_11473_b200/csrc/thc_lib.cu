@@ -1,0 +1,646 @@
+// C ABI of the THC-RR-CCSD projected doubles residual library (include/thc.h) and the evaluation plan.
+//
+// The plan is PAPER.md Algorithms 1, 2, 3, 6, 7, 8 (lines 5-10) and 9 re-blocked for one B200:
+//   * every contraction over an orbital, Cholesky or grid index is a call of the FP64 DMMA GEMM (thc_gemm.cuh),
+//     batched over Cholesky vectors / grid rows so that one launch covers a whole block;
+//   * Hadamard products are either fused into a GEMM epilogue (Z .* E^L, Alg.8 line 7 l.792; E .* V, Alg.7
+//     lines 14/18 l.757-763) or done by the HBM-streaming kernels of thc_kernels.cuh;
+//   * per-P NP x NP Hadamards of Alg.7 line 6 (l.743) and Alg.6 line 1 (l.683) are never materialised: the o x NP
+//     factor is row-scaled instead (B^{YZ} = v^{XY} o^{XZ} T^{YZ}  ->  (Xo .* v_X) Z (Xv .* o_X)^T);
+//   * Alg.6 line 11 (l.714) runs on the FP64 FMA pipe (triple_product_kernel).
+// Notation: P,Q,R amplitude grid (paper W,X,Y,Z), I,J ERI grid, L Cholesky index (paper A); see DESIGN.md.
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include "thc_host.cuh"
+
+using thc::i64;
+using thc::Ctx;
+using thc::Gemm;
+
+namespace {
+
+struct Inputs {
+  const double *Xo, *Xv, *Z, *B_ov, *B_oo, *B_vv, *Y, *V, *eps;
+};
+struct Outputs {
+  double* R;
+  double* terms[6];   // s1 s2 s3 s6 s7 s9 (NULL -> scratch)
+  double* xi_oo;
+  double* xi_vv;
+};
+
+inline i64 pad_to(i64 x, i64 m) { return (x + m - 1) / m * m; }
+
+// The whole residual evaluation.  Runs either for real or dry (workspace sizing); both take identical branches.
+void plan_residual(Ctx& c, const Inputs& in, const Outputs& out) {
+  thc_handle* h = c.h;
+  thc::Arena& ar = c.ar;
+  const i64 o = h->o, v = h->v, NL = h->NL, NP = h->NP, NX = h->NX;
+  const i64 NP2 = NP * NP, ov = o * v;
+  const int mask = h->term_mask ? h->term_mask : THC_TERM_ALL;
+  const bool do_s1 = mask & THC_TERM_S1, do_s2 = mask & THC_TERM_S2, do_s3 = mask & THC_TERM_S3;
+  const bool do_s6 = mask & THC_TERM_S6, do_s7 = mask & THC_TERM_S7, do_s9 = mask & THC_TERM_S9;
+  const double* Yo = in.Y;
+  const double* Yv = in.Y + o * NX;
+
+  // ---- persistent buffers -----------------------------------------------------------------------------------------
+  double* term[6];
+  for (int k = 0; k < 6; k++) term[k] = out.terms[k] ? out.terms[k] : ar.alloc(NP2);
+  double *s1 = term[0], *s2 = term[1], *s3 = term[2], *s6 = term[3], *s7 = term[4], *s9 = term[5];
+  double* xi_oo = out.xi_oo ? out.xi_oo : ar.alloc(o * o);
+  double* xi_vv = out.xi_vv ? out.xi_vv : ar.alloc(v * v);
+  double* XoT = ar.alloc(NP * o);
+  double* XvT = ar.alloc(NP * v);
+  double* YoT = ar.alloc(NX * o);
+  double* YvT = ar.alloc(NX * v);
+  double *omat = ar.alloc(NP2), *vmat = ar.alloc(NP2), *wmat = ar.alloc(NP2), *Kmat = ar.alloc(NP2), *C3 = ar.alloc(NP2);
+  double *Aa = ar.alloc(NL * NP), *Dm = ar.alloc(NL * NP);
+
+  // ---- H0: transposed factors and grams (Alg.1 l.481-485) ------------------------------------------------------------
+  c.transpose(in.Xo, XoT, o, NP);
+  c.transpose(in.Xv, XvT, v, NP);
+  c.transpose(Yo, YoT, o, NX);
+  c.transpose(Yv, YvT, v, NX);
+  c.gemm(Gemm(XoT, o, 'K', XoT, o, 'K', omat, NP, NP, NP, o));
+  c.gemm(Gemm(XvT, v, 'K', XvT, v, 'K', vmat, NP, NP, NP, v));
+  c.hadamard(omat, vmat, wmat, NP2);                                         // w = o .* v
+  c.gemm(Gemm(wmat, NP, 'K', in.Z, NP, 'K', Kmat, NP, NP, NP, NP));           // K = w Z   (Z symmetric)
+  c.fill(C3, NP2, 0.0);
+  c.fill(s1, NP2, 0.0);
+  c.fill(xi_oo, o * o, 0.0);
+  c.fill(xi_vv, v * v, 0.0);
+
+  // ---- L-block loop: Alg.1 + Alg.3 (H1-H4) and Alg.2 + Alg.8 (H5-H6) fused over the Cholesky index (l.238) ---------
+  const bool need_ladder = do_s1 || do_s3;
+  const bool need_ring = do_s2 || do_s9;
+  for (i64 L0 = 0; L0 < NL; L0 += h->bL) {
+    const i64 nl = std::min<i64>(h->bL, NL - L0);
+    const i64 m0 = ar.mark();
+    if (need_ladder) {
+      double* T1T = ar.alloc(NP * nl * o);
+      double* T2T = ar.alloc(NP * nl * v);
+      double *Mo = ar.alloc(nl * NP2), *Mv = ar.alloc(nl * NP2);
+      // H1: T1T[P][(l,j)] = sum_i Xo[i,P] B^l_ij ;  Mo^l[P][Q] = sum_j T1T[P][(l,j)] Xo[j,Q]      (Alg.1 lines 6-7)
+      c.gemm(Gemm(XoT, o, 'K', in.B_oo + L0 * o * o, o, 'K', T1T, nl * o, NP, nl * o, o));
+      c.gemm(Gemm(T1T, nl * o, 'K', XoT, o, 'K', Mo, NP, NP, NP, o).batch(nl, o, 0, NP2));
+      // H2: same with the vv block                                                                  (Alg.1 lines 10-11)
+      c.gemm(Gemm(XvT, v, 'K', in.B_vv + L0 * v * v, v, 'K', T2T, nl * v, NP, nl * v, v));
+      c.gemm(Gemm(T2T, nl * v, 'K', XvT, v, 'K', Mv, NP, NP, NP, v).batch(nl, v, 0, NP2));
+      // H3: C^l = v .* Mo^l - o .* Mv^l (in place over Mo);  C3 += Mo^l .* Mv^l                   (Alg.1 l.8,12,13; Alg.3 l.7)
+      c.combine(Mo, Mv, omat, vmat, C3, NP2, nl);
+      if (do_s1) {
+        // H4: D^l = C^l Z ;  s1 += sum_l D^l C^l^T                                                   (Alg.1 lines 14-15)
+        double* D = Mv;   // Mv is dead after the combine
+        c.gemm(Gemm(Mo, NP, 'K', in.Z, NP, 'K', D, NP, nl * NP, NP, NP));
+        c.gemm(Gemm(D, NP, 'K', Mo, NP, 'K', s1, NP, NP, NP, NP).kbatch(nl, NP2, NP2).ab(1.0, 1.0));
+      }
+      ar.release(m0);
+    }
+    if (need_ring) {
+      // H5: TT[Q][(l,i)] = sum_a Xv[a,Q] B^l_ia ;  a^l_P = sum_i Xo[i,P] TT[P][(l,i)]              (Alg.8 line 5 l.788)
+      double* TT = ar.alloc(NP * nl * o);
+      c.gemm(Gemm(XvT, v, 'K', in.B_ov + L0 * ov, v, 'K', TT, nl * o, NP, nl * o, v));
+      c.rowdot(XoT, o, TT, o, nl * o, Aa + L0 * NP, NP, nl, NP, o);
+      // W^l = Z .* E^l,  E^l[P][Q] = sum_i Xo[i,P] TT[Q][(l,i)]                                     (Alg.8 lines 6-7)
+      double* W = ar.alloc(nl * NP2);
+      c.gemm(Gemm(XoT, o, 'K', TT, nl * o, 'K', W, NP, NP, NP, o).batch(nl, 0, o, NP2).aux(in.Z, NP, 0));
+      double* ZA = ar.alloc(nl * NP);
+      c.gemm(Gemm(Aa + L0 * NP, NP, 'K', in.Z, NP, 'K', ZA, NP, nl, NP, NP));
+      // H6: D^l_ia = sum_PQ Xo[i,Q] Xv[a,P] N^l_PQ,  N^l = 2 diag(Z a^l) - W^l                      (Alg.8 line 8 l.794)
+      double* G1 = ar.alloc(o * nl * NP);
+      c.gemm(Gemm(in.Xo, NP, 'K', W, NP, 'K', G1, nl * NP, o, nl * NP, NP));
+      c.qm(G1, in.Xo, ZA, o, nl, NP);
+      double* Dia = ar.alloc(nl * ov);
+      c.gemm(Gemm(G1, nl * NP, 'K', in.Xv, NP, 'K', Dia, v, o, v, NP).batch(nl, NP, 0, ov));
+      // xi_ij += sum_a B^l_ia D^l_ja ;  xi_ab -= sum_i D^l_ia B^l_ib                               (Alg.8 lines 9-10; Eqs.39-40)
+      c.gemm(Gemm(in.B_ov + L0 * ov, v, 'K', Dia, v, 'K', xi_oo, o, o, o, v).kbatch(nl, ov, ov).ab(1.0, 1.0));
+      c.gemm(Gemm(Dia, v, 'M', in.B_ov + L0 * ov, v, 'N', xi_vv, v, v, v, nl * o).ab(-1.0, 1.0));
+      // d^l_P = sum_ia Xo[i,P] Xv[a,P] D^l_ia                                                         (Alg.2 lines 8, 12)
+      double* DX = ar.alloc(nl * o * NP);
+      c.gemm(Gemm(Dia, v, 'K', XvT, v, 'K', DX, NP, nl * o, NP, v));
+      c.coldot(in.Xo, NP, DX, o * NP, NP, Dm + L0 * NP, NP, nl, NP, o);
+      ar.release(m0);
+    }
+  }
+
+  // ---- H7: s2 = A A^T + Dm A^T + A Dm^T  (Alg.2 line 13 l.559; rows of Aa/Dm are Cholesky vectors) --------------------
+  if (do_s2) {
+    const i64 m0 = ar.mark();
+    double* AD = ar.alloc(NL * NP);
+    c.axpby(Aa, Dm, 1.0, 1.0, AD, NL * NP);
+    c.gemm(Gemm(AD, NP, 'M', Aa, NP, 'N', s2, NP, NP, NP, NL));
+    c.gemm(Gemm(Aa, NP, 'M', Dm, NP, 'N', s2, NP, NP, NP, NL).ab(1.0, 1.0));
+    ar.release(m0);
+  } else {
+    c.fill(s2, NP2, 0.0);
+  }
+
+  // ---- H8: Alg.3 tail and Alg.9 ------------------------------------------------------------------------------------
+  if (do_s3) {
+    // s3 = -(K C3^T + C3 K^T)                                                                        (Alg.3 line 12 l.601)
+    const i64 m0 = ar.mark();
+    double* P3 = ar.alloc(NP2);
+    c.gemm(Gemm(Kmat, NP, 'K', C3, NP, 'K', P3, NP, NP, NP, NP));
+    c.symmetrize(P3, s3, NP, -1.0);
+    ar.release(m0);
+  } else {
+    c.fill(s3, NP2, 0.0);
+  }
+  if (do_s9) {
+    // F'_oo = diag(eps_o) + xi_oo, F'_vv = diag(eps_v) + xi_vv; o~ = Xo^T F'_oo^T.. (Alg.9 lines 5-10 l.823-839)
+    const i64 m0 = ar.mark();
+    double *FooT = ar.alloc(o * o), *Fvv = ar.alloc(v * v);
+    double *CoT = ar.alloc(NP * o), *DvT = ar.alloc(NP * v), *otil = ar.alloc(NP2), *vtil = ar.alloc(NP2);
+    double *E9 = ar.alloc(NP2), *P9 = ar.alloc(NP2);
+    c.fock(in.eps, xi_oo, xi_vv, FooT, Fvv, o, v);
+    c.gemm(Gemm(XoT, o, 'K', FooT, o, 'K', CoT, o, NP, o, o));         // CoT[P][i] = sum_j Xo[j,P] F'[j][i]
+    c.gemm(Gemm(XoT, o, 'K', CoT, o, 'K', otil, NP, NP, NP, o));       // o~[P][Q] = sum_i Xo[i,P] C_i^Q
+    c.gemm(Gemm(XvT, v, 'K', Fvv, v, 'K', DvT, v, NP, v, v));          // DvT[P][a] = sum_b Xv[b,P] F'[a][b]
+    c.gemm(Gemm(XvT, v, 'K', DvT, v, 'K', vtil, NP, NP, NP, v));
+    c.had2_diff(omat, vtil, otil, vmat, E9, NP2);                       // E = o .* v~ - o~ .* v
+    c.gemm(Gemm(E9, NP, 'K', Kmat, NP, 'K', P9, NP, NP, NP, NP));       // E K^T
+    c.symmetrize(P9, s9, NP, 1.0);
+    ar.release(m0);
+  } else {
+    c.fill(s9, NP2, 0.0);
+  }
+
+  // ---- H10: Alg.7, ring-type T2^2 terms with THC ERIs (Eqs.35-37 l.261-271; prefactor 1/2, R2) -----------
+  if (do_s7) {
+    const i64 m0 = ar.mark();
+    double *Rb = ar.alloc(NP * ov), *Sb = ar.alloc(NP * ov), *C7 = ar.alloc(NP * NX);
+    // pass 1 (Alg.7 lines 3-7): S^P = -(Xo .* v_P) Z (Xv .* o_P)^T ;  R^P = 2 (Xo .* K_P) Xv^T + S^P
+    const i64 bA = std::min<i64>(NP, h->bP7 * 16);
+    for (i64 P0 = 0; P0 < NP; P0 += bA) {
+      const i64 npb = std::min<i64>(bA, NP - P0), m1 = ar.mark();
+      double *XoV = ar.alloc(npb * o * NP), *SZ = ar.alloc(npb * o * NP);
+      c.rowscale(in.Xo, NP, vmat + P0 * NP, NP, nullptr, 1.0, XoV, npb, o, NP);
+      c.gemm(Gemm(XoV, NP, 'K', in.Z, NP, 'K', SZ, NP, npb * o, NP, NP));
+      c.rowscale_inplace(SZ, omat + P0 * NP, NP, -1.0, npb, o, NP);
+      c.gemm(Gemm(SZ, NP, 'K', in.Xv, NP, 'K', Sb + P0 * ov, v, npb * o, v, NP));
+      c.rowscale(in.Xo, NP, Kmat + P0 * NP, NP, SZ, 2.0, XoV, npb, o, NP);         // RA (reuses XoV)
+      c.gemm(Gemm(XoV, NP, 'K', in.Xv, NP, 'K', Rb + P0 * ov, v, npb * o, v, NP));
+      ar.release(m1);
+    }
+    // pass 2 (lines 9-19): per P, E = Yo^T R^P Yv, F = E .* V, G^P = Yo F^T Yv^T; rows of s7 from G R^T and G~ S^T
+    for (i64 P0 = 0; P0 < NP; P0 += h->bP7) {
+      const i64 npb = std::min<i64>(h->bP7, NP - P0), m1 = ar.mark();
+      double *RYT = ar.alloc(npb * NX * o), *EF = ar.alloc(npb * NX * NX), *FYT = ar.alloc(npb * o * NX), *Gb = ar.alloc(npb * ov);
+      for (int pass = 0; pass < 2; pass++) {
+        const double* src = pass == 0 ? Rb : Sb;
+        c.gemm(Gemm(YvT, v, 'K', src + P0 * ov, v, 'K', RYT, o, NX, o, v).batch(npb, 0, ov, NX * o));
+        if (pass == 0) c.rowdot(YoT, o, RYT, NX * o, o, C7 + P0 * NX, NX, npb, NX, o);     // line 9
+        c.gemm(Gemm(YoT, o, 'K', RYT, o, 'K', EF, NX, NX, NX, o).batch(npb, 0, NX * o, NX * NX).aux(in.V, NX, 0));
+        c.gemm(Gemm(Yo, NX, 'K', EF, NX, 'K', FYT, NX, o, NX, NX).batch(npb, 0, NX * NX, o * NX));
+        c.gemm(Gemm(FYT, NX, 'K', Yv, NX, 'K', Gb, v, npb * o, v, NX));
+        c.gemm(Gemm(Gb, ov, 'K', src, ov, 'K', s7 + P0 * NP, NP, npb, NP, ov).ab(pass == 0 ? -0.5 : 0.5, pass == 0 ? 0.0 : 1.0));
+      }
+      ar.release(m1);
+    }
+    // line 10 + first part of line 22: s7 += C7 V C7^T
+    double* CV = ar.alloc(NP * NX);
+    c.gemm(Gemm(C7, NX, 'K', in.V, NX, 'K', CV, NX, NP, NX, NX));
+    c.gemm(Gemm(CV, NX, 'K', C7, NX, 'K', s7, NP, NP, NP, NX).ab(1.0, 1.0));
+    ar.release(m0);
+  } else {
+    c.fill(s7, NP2, 0.0);
+  }
+
+  // ---- H9: Alg.6, ladder-type T2^2 terms with THC ERIs (Eq.34 l.254) -------------------------------------------------
+  if (do_s6) {
+    const i64 m0 = ar.mark();
+    const i64 NPp = pad_to(NP, thc::TP_RT);
+    // line 1: A3[Q][i][a] = sum_S Z[Q,S] Xo[i,S] Xv[a,S]
+    double* A3 = ar.alloc(NP * ov);
+    const i64 bA = std::min<i64>(NP, h->bP7 * 16);
+    for (i64 P0 = 0; P0 < NP; P0 += bA) {
+      const i64 npb = std::min<i64>(bA, NP - P0), m1 = ar.mark();
+      double* ZX = ar.alloc(npb * o * NP);
+      c.rowscale(in.Xo, NP, in.Z + P0 * NP, NP, nullptr, 1.0, ZX, npb, o, NP);
+      c.gemm(Gemm(ZX, NP, 'K', in.Xv, NP, 'K', A3 + P0 * ov, v, npb * o, v, NP));
+      ar.release(m1);
+    }
+    for (i64 P0 = 0; P0 < NP; P0 += h->bX) {
+      const i64 npb = std::min<i64>(h->bX, NP - P0), m1 = ar.mark();
+      const i64 bXp = pad_to(npb, thc::TP_PT);
+      // lines 4-5: Cc[p][(q,i)] = sum_a Xv[a,P0+p] A3[q][i][a] ;  Dd[p][(q,a)] = sum_i Xo[i,P0+p] A3[q][i][a]
+      double *Cc = ar.alloc(npb * NP * o), *Dd = ar.alloc(npb * NP * v), *H = ar.alloc(bXp * NPp * NPp);
+      c.gemm(Gemm(XvT + P0 * v, v, 'K', A3, v, 'K', Cc, NP * o, npb, NP * o, v));
+      c.gemm(Gemm(XoT + P0 * o, o, 'K', A3, v, 'N', Dd, NP * v, npb, v, o).batch(NP, 0, ov, v));
+      bool first = true;
+      for (i64 I0 = 0; I0 < NX; I0 += h->bI) {
+        const i64 ni = std::min<i64>(h->bI, NX - I0), m2 = ar.mark();
+        // line 2/7: BI[I][i][a] = sum_J V[I,J] Yo[i,J] Yv[a,J]
+        double *VY = ar.alloc(ni * o * NX), *BI = ar.alloc(ni * ov), *GXT = ar.alloc(ni * NP * o), *Gt = ar.alloc(ni * NPp * NPp);
+        double *Eb = ar.alloc(ni * bXp * NPp), *Fb = ar.alloc(ni * bXp * NPp);
+        c.rowscale(Yo, NX, in.V + I0 * NX, NX, nullptr, 1.0, VY, ni, o, NX);
+        c.gemm(Gemm(VY, NX, 'K', Yv, NX, 'K', BI, v, ni * o, v, NX));
+        // line 10: G_I[q][r] = sum_ia Xo[i,q] Xv[a,r] BI[I][i][a]
+        c.gemm(Gemm(XvT, v, 'K', BI, v, 'K', GXT, o, NP, o, v).batch(ni, 0, ov, NP * o));
+        c.gemm(Gemm(XoT, o, 'K', GXT, o, 'K', Gt, NPp, NP, NP, o).batch(ni, 0, NP * o, NPp * NPp));
+        // lines 8-9: E_I[p][q] = sum_i Cc[p][(q,i)] Yo[i,I] ;  F_I[p][r] = sum_a Dd[p][(r,a)] Yv[a,I]
+        c.gemm(Gemm(YoT + I0 * o, o, 'K', Cc, o, 'K', Eb, bXp * NPp, ni, NP, o).batch(npb, 0, NP * o, NPp));
+        c.gemm(Gemm(YvT + I0 * v, v, 'K', Dd, v, 'K', Fb, bXp * NPp, ni, NP, v).batch(npb, 0, NP * v, NPp));
+        // line 11
+        c.triple_product(Eb, Fb, Gt, H, ni, bXp, NPp, first ? 0 : 1);
+        first = false;
+        ar.release(m2);
+      }
+      // lines 14-15: I^P_ia = sum_QR Xo[i,R] Xv[a,Q] H[P][Q][R] ;  s6[P][S] = sum_ia Xo[i,S] Xv[a,S] I^P_ia
+      double *HT1 = ar.alloc(npb * NP * o), *Iia = ar.alloc(npb * ov), *IX = ar.alloc(npb * o * NP);
+      c.gemm(Gemm(H, NPp, 'K', in.Xo, NP, 'K', HT1, o, NP, o, NP).batch(npb, NPp * NPp, 0, NP * o));
+      c.gemm(Gemm(HT1, o, 'M', in.Xv, NP, 'K', Iia, v, o, v, NP).batch(npb, NP * o, 0, ov));
+      c.gemm(Gemm(Iia, v, 'K', XvT, v, 'K', IX, NP, npb * o, NP, v));
+      c.coldot(in.Xo, NP, IX, o * NP, NP, s6 + P0 * NP, NP, npb, NP, o);
+      ar.release(m1);
+    }
+    ar.release(m0);
+  } else {
+    c.fill(s6, NP2, 0.0);
+  }
+
+  // ---- H11 ---------------------------------------------------------------------------------------------------------
+  if (out.R) c.sum6(term, out.R, NP2);
+}
+
+// Correlation energy, factorised (R7):  E = sum_L [ 2 a^L . Z a^L - sum_PQ Z_PQ E^L_PQ E^L_QP ],
+// a^L, E^L as in Alg.8 lines 5-6 (l.788-790).  Result in E_dev[0] (device).
+void plan_energy(Ctx& c, const double* Xo, const double* Xv, const double* Z, const double* B_ov, double* E_dev) {
+  thc_handle* h = c.h;
+  thc::Arena& ar = c.ar;
+  const i64 o = h->o, v = h->v, NL = h->NL, NP = h->NP, NP2 = NP * NP, ov = o * v;
+  const i64 nblk = (NL + h->bL - 1) / h->bL;
+  double *XoT = ar.alloc(NP * o), *XvT = ar.alloc(NP * v), *Aa = ar.alloc(NL * NP), *ZA = ar.alloc(NL * NP);
+  double* Eblk = ar.alloc(nblk);
+  c.transpose(Xo, XoT, o, NP);
+  c.transpose(Xv, XvT, v, NP);
+  i64 blk = 0;
+  for (i64 L0 = 0; L0 < NL; L0 += h->bL, blk++) {
+    const i64 nl = std::min<i64>(h->bL, NL - L0), m0 = ar.mark();
+    double *TT = ar.alloc(NP * nl * o), *El = ar.alloc(nl * NP2);
+    const i64 nz = c.zee_blocks(NP, nl);
+    double* part = ar.alloc(nz);
+    c.gemm(Gemm(XvT, v, 'K', B_ov + L0 * ov, v, 'K', TT, nl * o, NP, nl * o, v));
+    c.rowdot(XoT, o, TT, o, nl * o, Aa + L0 * NP, NP, nl, NP, o);
+    c.gemm(Gemm(XoT, o, 'K', TT, nl * o, 'K', El, NP, NP, NP, o).batch(nl, 0, o, NP2));
+    c.zee_partial(Z, El, NP, nl, part);
+    c.final_sum(part, nz, -1.0, nullptr, 0, 0.0, Eblk + blk, 0);
+    ar.release(m0);
+  }
+  c.gemm(Gemm(Aa, NP, 'K', Z, NP, 'K', ZA, NP, NL, NP, NP));
+  const i64 nd = c.dot_blocks(NL * NP);
+  double* part2 = ar.alloc(nd);
+  c.dot_partial(Aa, ZA, NL * NP, part2);
+  c.final_sum(Eblk, nblk, 1.0, part2, nd, 2.0, E_dev, 0);
+}
+
+// ---- dry runs: workspace sizes for the three entry points ------------------------------------------------------------
+struct Need { i64 arena_bytes, splitk_doubles; i64 total() const { return arena_bytes + (splitk_doubles * 8 + 255) / 256 * 256 + 256; } };
+
+Need dry_residual(thc_handle* h) {
+  Ctx c{h}; c.dry = true; c.ar.dry = true;
+  Inputs in{}; Outputs out{};
+  plan_residual(c, in, out);
+  return Need{c.ar.peak, c.splitk_need};
+}
+Need dry_energy(thc_handle* h) {
+  Ctx c{h}; c.dry = true; c.ar.dry = true;
+  double* e = c.ar.alloc(1);
+  plan_energy(c, nullptr, nullptr, nullptr, nullptr, e);
+  return Need{c.ar.peak, c.splitk_need};
+}
+i64 input_doubles(const thc_handle* h, i64 sizes[9]) {
+  const i64 o = h->o, v = h->v, NL = h->NL, NP = h->NP, NX = h->NX;
+  const i64 s[9] = {o * NP, v * NP, NP * NP, NL * o * v, NL * o * o, NL * v * v, (o + v) * NX, NX * NX, o + v};
+  i64 tot = 0;
+  for (int k = 0; k < 9; k++) { sizes[k] = s[k]; tot += (s[k] * 8 + 255) / 256 * 256; }
+  return tot;   // bytes
+}
+i64 need_device(thc_handle* h) { return std::max<i64>(dry_residual(h).total(), dry_energy(h).total()); }
+i64 need_host(thc_handle* h) {
+  i64 sz[9];
+  Need r = dry_residual(h), e = dry_energy(h);
+  i64 staging = input_doubles(h, sz) + (h->NP * h->NP * 8 + 255) / 256 * 256 + 256;
+  return staging + std::max<i64>(r.total(), e.total());
+}
+
+bool bad_ptr(const void* p) { return p == nullptr || (reinterpret_cast<uintptr_t>(p) & 7) != 0; }
+
+// Make sure a workspace of `bytes` exists (library-owned unless the caller provided one).
+int ensure_workspace(thc_handle* h, i64 bytes) {
+  if (h->ws && h->ws_bytes >= bytes) return THC_OK;
+  if (h->ws && !h->ws_owned) return THC_ERR_NO_MEMORY;     // caller's buffer is too small
+  if (h->ws) { cudaStreamSynchronize(h->stream); cudaFree(h->ws); h->ws = nullptr; h->ws_bytes = 0; }
+  void* p = nullptr;
+  cudaError_t e = cudaMalloc(&p, (size_t)bytes);
+  if (e != cudaSuccess) { h->last_cuda = (int)e; cudaGetLastError(); return THC_ERR_NO_MEMORY; }
+  h->ws = p; h->ws_bytes = bytes; h->ws_owned = true;
+  return THC_OK;
+}
+
+// Real-run context over [base, base + bytes): split-K scratch first, arena after it.
+int make_ctx(Ctx& c, thc_handle* h, char* base, i64 bytes, const Need& need) {
+  if (need.total() > bytes) return THC_ERR_NO_MEMORY;
+  c.h = h; c.dry = false;
+  uintptr_t b = (reinterpret_cast<uintptr_t>(base) + 255) / 256 * 256;
+  c.splitk = reinterpret_cast<double*>(b);
+  c.splitk_cap = need.splitk_doubles;
+  i64 sk = (need.splitk_doubles * 8 + 255) / 256 * 256;
+  c.ar.base = reinterpret_cast<char*>(b) + sk;
+  c.ar.cap = bytes - sk - (i64)(b - reinterpret_cast<uintptr_t>(base));
+  c.ar.dry = false;
+  return THC_OK;
+}
+
+struct DeviceGuard {
+  int prev = -1; bool ok = true;
+  explicit DeviceGuard(int dev) { if (cudaGetDevice(&prev) != cudaSuccess) ok = false; else if (prev != dev) ok = cudaSetDevice(dev) == cudaSuccess; }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+int run_residual(thc_handle* h, char* base, i64 bytes, const Inputs& in, const Outputs& out) {
+  Need need = dry_residual(h);
+  Ctx c{h};
+  int st = make_ctx(c, h, base, bytes, need);
+  if (st != THC_OK) return st;
+  plan_residual(c, in, out);
+  if (c.ar.overflow) return THC_ERR_NO_MEMORY;
+  return c.status;
+}
+int run_energy(thc_handle* h, char* base, i64 bytes, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
+               double* E_host) {
+  Need need = dry_energy(h);
+  Ctx c{h};
+  int st = make_ctx(c, h, base, bytes, need);
+  if (st != THC_OK) return st;
+  double* e = c.ar.alloc(1);
+  plan_energy(c, Xo, Xv, Z, B_ov, e);
+  if (c.ar.overflow) return THC_ERR_NO_MEMORY;
+  if (c.status != THC_OK) return c.status;
+  c.check(cudaMemcpyAsync(E_host, e, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+  c.check(cudaStreamSynchronize(h->stream));
+  return c.status;
+}
+
+}  // namespace
+
+// =====================================================================================================================
+// C ABI
+// =====================================================================================================================
+extern "C" {
+
+int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int64_t NX, const thc_options* opt) {
+  if (!hp) return THC_ERR_INVALID_ARG;
+  *hp = nullptr;
+  if (o <= 0 || v <= 0 || NL <= 0 || NP <= 0 || NX <= 0) return THC_ERR_INVALID_ARG;
+  if (opt && (opt->bL < 0 || opt->bP7 < 0 || opt->bX < 0 || opt->bI < 0 || opt->workspace_bytes_max < 0)) return THC_ERR_INVALID_ARG;
+  const int64_t lim = (int64_t)1 << 31;
+  if (o >= lim || v >= lim || NL >= lim || NP >= lim || NX >= lim) return THC_ERR_OVERFLOW;
+  // largest single buffers must stay below 2^60 bytes and GEMM extents below 2^31
+  const long double big = (long double)NL * v * v;
+  if (big * 8 > 1e18L || (long double)NP * NP * std::max<i64>(o, v) > 9e18L) return THC_ERR_OVERFLOW;
+  if ((long double)NP * o * 64 >= (long double)lim || (long double)NX * NX >= 9e18L) return THC_ERR_OVERFLOW;
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); return THC_ERR_NO_DEVICE; }
+  int dev = (opt && opt->device >= 0) ? opt->device : -1;
+  if (dev < 0 && cudaGetDevice(&dev) != cudaSuccess) return THC_ERR_NO_DEVICE;
+  if (dev >= ndev) return THC_ERR_INVALID_ARG;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return THC_ERR_NO_DEVICE;
+  if (prop.major != 10) return THC_ERR_NO_DEVICE;     // sm_100a binary only
+
+  thc_handle* h = new (std::nothrow) thc_handle();
+  if (!h) return THC_ERR_NO_MEMORY;
+  h->o = o; h->v = v; h->NL = NL; h->NP = NP; h->NX = NX;
+  h->term_mask = opt ? (opt->term_mask & THC_TERM_ALL) : 0;
+  h->device = dev; h->sms = prop.multiProcessorCount;
+  h->stream = nullptr; h->ws = nullptr; h->ws_bytes = 0; h->ws_owned = false;
+  h->launches = 0; h->last_cuda = 0; h->smem_configured = false;
+
+  // block sizes: defaults, then shrink until the plan fits the cap
+  h->bL = std::min<int64_t>(NL, (opt && opt->bL) ? opt->bL : 32);
+  const int64_t p7_auto = std::max<int64_t>(1, ((int64_t)2 << 30) / (NX * NX * 8));
+  h->bP7 = std::min<int64_t>(NP, (opt && opt->bP7) ? opt->bP7 : p7_auto);
+  h->bX = std::min<int64_t>(pad_to(NP, 16), (opt && opt->bX) ? pad_to(opt->bX, 16) : pad_to(NP, 16));
+  h->bI = std::min<int64_t>(NX, (opt && opt->bI) ? opt->bI : 64);
+  int64_t cap = opt ? opt->workspace_bytes_max : 0;
+  if (cap == 0) {
+    DeviceGuard g(dev);
+    size_t fr = 0, tot = 0;
+    if (!g.ok || cudaMemGetInfo(&fr, &tot) != cudaSuccess) { delete h; return THC_ERR_CUDA; }
+    cap = (int64_t)(0.75 * (double)fr);
+  }
+  const bool fix_bX = opt && opt->bX, fix_bI = opt && opt->bI, fix_bP7 = opt && opt->bP7, fix_bL = opt && opt->bL;
+  for (;;) {
+    h->need_bytes = need_device(h);
+    if (h->need_bytes <= cap) break;
+    if (!fix_bX && h->bX > 64) h->bX = pad_to(h->bX / 2, 16);
+    else if (!fix_bP7 && h->bP7 > 1) h->bP7 = h->bP7 / 2;
+    else if (!fix_bL && h->bL > 4) h->bL = h->bL / 2;
+    else if (!fix_bI && h->bI > 16) h->bI = h->bI / 2;
+    else if (!fix_bX && h->bX > 16) h->bX = pad_to(h->bX / 2, 16);
+    else if (!fix_bL && h->bL > 1) h->bL = h->bL / 2;
+    else { delete h; return THC_ERR_NO_MEMORY; }
+  }
+  *hp = h;
+  return THC_OK;
+}
+
+int thc_destroy(thc_handle* h) {
+  if (!h) return THC_ERR_INVALID_ARG;
+  if (h->ws && h->ws_owned) {
+    DeviceGuard g(h->device);
+    cudaStreamSynchronize(h->stream);
+    cudaFree(h->ws);
+  }
+  delete h;
+  return THC_OK;
+}
+
+int64_t thc_workspace_bytes(const thc_handle* h) { return h ? h->need_bytes : (int64_t)THC_ERR_INVALID_ARG; }
+int64_t thc_workspace_bytes_host(const thc_handle* h) { return h ? need_host(const_cast<thc_handle*>(h)) : (int64_t)THC_ERR_INVALID_ARG; }
+
+int thc_set_workspace(thc_handle* h, void* device_ptr, int64_t bytes) {
+  if (!h || !device_ptr || bytes <= 0) return THC_ERR_INVALID_ARG;
+  if (h->ws && h->ws_owned) {
+    DeviceGuard g(h->device);
+    cudaStreamSynchronize(h->stream);
+    cudaFree(h->ws);
+  }
+  h->ws = device_ptr; h->ws_bytes = bytes; h->ws_owned = false;
+  return THC_OK;
+}
+
+int thc_set_stream(thc_handle* h, void* cuda_stream) {
+  if (!h) return THC_ERR_INVALID_ARG;
+  h->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+  return THC_OK;
+}
+
+int thc_get_blocks(const thc_handle* h, int64_t out[4]) {
+  if (!h || !out) return THC_ERR_INVALID_ARG;
+  out[0] = h->bL; out[1] = h->bP7; out[2] = h->bX; out[3] = h->bI;
+  return THC_OK;
+}
+
+int thc_residual_terms(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
+                       const double* B_oo, const double* B_vv, const double* Y, const double* V, const double* eps,
+                       double* R, double* const terms[6], double* xi_oo, double* xi_vv) {
+  if (!h) return THC_ERR_INVALID_ARG;
+  if (bad_ptr(Xo) || bad_ptr(Xv) || bad_ptr(Z) || bad_ptr(B_ov) || bad_ptr(B_oo) || bad_ptr(B_vv) || bad_ptr(Y) ||
+      bad_ptr(V) || bad_ptr(eps))
+    return THC_ERR_INVALID_ARG;
+  Inputs in{Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps};
+  Outputs out{};
+  out.R = R;
+  bool any = R != nullptr;
+  for (int k = 0; k < 6; k++) { out.terms[k] = terms ? terms[k] : nullptr; any = any || out.terms[k]; }
+  out.xi_oo = xi_oo; out.xi_vv = xi_vv;
+  if (!any && !xi_oo && !xi_vv) return THC_ERR_INVALID_ARG;
+  if ((R && bad_ptr(R)) || (xi_oo && bad_ptr(xi_oo)) || (xi_vv && bad_ptr(xi_vv))) return THC_ERR_INVALID_ARG;
+  DeviceGuard g(h->device);
+  if (!g.ok) return THC_ERR_CUDA;
+  int st = ensure_workspace(h, h->need_bytes);
+  if (st != THC_OK) return st;
+  return run_residual(h, static_cast<char*>(h->ws), h->ws_bytes, in, out);
+}
+
+int thc_residual(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
+                 const double* B_oo, const double* B_vv, const double* Y, const double* V, const double* eps, double* R) {
+  if (!R) return THC_ERR_INVALID_ARG;
+  return thc_residual_terms(h, Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps, R, nullptr, nullptr, nullptr);
+}
+
+int thc_energy(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov, double* E_host) {
+  if (!h || bad_ptr(Xo) || bad_ptr(Xv) || bad_ptr(Z) || bad_ptr(B_ov) || !E_host) return THC_ERR_INVALID_ARG;
+  DeviceGuard g(h->device);
+  if (!g.ok) return THC_ERR_CUDA;
+  int st = ensure_workspace(h, h->need_bytes);
+  if (st != THC_OK) return st;
+  return run_energy(h, static_cast<char*>(h->ws), h->ws_bytes, Xo, Xv, Z, B_ov, E_host);
+}
+
+int thc_residual_host(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
+                      const double* B_oo, const double* B_vv, const double* Y, const double* V, const double* eps,
+                      double* R_host, double* E_host) {
+  if (!h || !R_host) return THC_ERR_INVALID_ARG;
+  const double* src[9] = {Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps};
+  for (int k = 0; k < 9; k++) if (bad_ptr(src[k])) return THC_ERR_INVALID_ARG;
+  DeviceGuard g(h->device);
+  if (!g.ok) return THC_ERR_CUDA;
+  const i64 need = need_host(h);
+  int st = ensure_workspace(h, need);
+  if (st != THC_OK) return st;
+  // staging area at the front of the workspace
+  i64 sz[9];
+  input_doubles(h, sz);
+  char* p = reinterpret_cast<char*>((reinterpret_cast<uintptr_t>(h->ws) + 255) / 256 * 256);
+  double* dev[9];
+  for (int k = 0; k < 9; k++) {
+    dev[k] = reinterpret_cast<double*>(p);
+    cudaError_t e = cudaMemcpyAsync(dev[k], src[k], (size_t)sz[k] * 8, cudaMemcpyHostToDevice, h->stream);
+    if (e != cudaSuccess) { h->last_cuda = (int)e; return THC_ERR_CUDA; }
+    p += (sz[k] * 8 + 255) / 256 * 256;
+  }
+  double* Rd = reinterpret_cast<double*>(p);
+  p += (h->NP * h->NP * 8 + 255) / 256 * 256;
+  const i64 rest = h->ws_bytes - (p - static_cast<char*>(h->ws));
+  Inputs in{dev[0], dev[1], dev[2], dev[3], dev[4], dev[5], dev[6], dev[7], dev[8]};
+  Outputs out{};
+  out.R = Rd;
+  st = run_residual(h, p, rest, in, out);
+  if (st != THC_OK) return st;
+  cudaError_t e = cudaMemcpyAsync(R_host, Rd, (size_t)h->NP * h->NP * 8, cudaMemcpyDeviceToHost, h->stream);
+  if (e != cudaSuccess) { h->last_cuda = (int)e; return THC_ERR_CUDA; }
+  if (E_host) {
+    st = run_energy(h, p, rest, dev[0], dev[1], dev[2], dev[3], E_host);   // synchronises
+    if (st != THC_OK) return st;
+  }
+  e = cudaStreamSynchronize(h->stream);
+  if (e != cudaSuccess) { h->last_cuda = (int)e; return THC_ERR_CUDA; }
+  return THC_OK;
+}
+
+int64_t thc_kernel_launches(const thc_handle* h) { return h ? h->launches : 0; }
+
+// SURVEY.md 8(a) / DESIGN.md section 7: straightforward GEMM order, FMA = 2 flop, no symmetry savings, the G
+// intermediates of Alg.6 counted once (re-computation per X-block is not algorithmic work).
+double thc_algorithmic_flops(const thc_handle* h) {
+  if (!h) return 0.0;
+  const double o = (double)h->o, v = (double)h->v, NL = (double)h->NL, NP = (double)h->NP, NX = (double)h->NX;
+  const double NP2 = NP * NP, NP3 = NP2 * NP, ov = o * v;
+  double f = 0.0;
+  f += 2 * (o + v) * NP2 + 2 * NP3;                                                    // H0
+  f += NL * (2 * o * o * NP + 2 * o * NP2);                                            // H1
+  f += NL * (2 * v * v * NP + 2 * v * NP2);                                            // H2
+  f += 5 * NL * NP2;                                                                   // H3
+  f += 4 * NL * NP3;                                                                   // H4
+  f += NL * (2 * ov * NP + 2 * o * NP2);                                               // H5
+  f += NL * (4 * o * NP2 + 2 * ov * NP + 2 * o * o * v + 2 * ov * v);                  // H6
+  f += 6 * NP2 * NL;                                                                   // H7
+  f += 4 * NP3 + 4 * (o + v) * NP2 + 2 * (o * o + v * v) * NP;                         // H8
+  f += 2 * ov * NP2 + 4 * ov * NP2;                                                    // H9 (a),(b): A3, C, D
+  f += 2 * ov * NX * NX + NX * (2 * ov * NP + 2 * o * NP2);                            // H9 B_ia^I and G
+  f += 2 * (o + v) * NP2 * NX;                                                         // H9 (c): E, F
+  f += 5 * NX * NP3;                                                                   // H9 (d): line 11
+  f += NP * (2 * o * NP2 + 4 * ov * NP);                                               // H9 (e)
+  f += NP * (2 * o * NP2 + 4 * ov * NP);                                               // H10 pass 1
+  f += 2 * NP * (4 * o * NX * NX + 4 * ov * NX);                                       // H10 pass 2 (R and S)
+  f += 4 * NP2 * ov + 2 * NP * NX * NX + 2 * NP2 * NX;                                 // H10 assembly
+  return f;
+}
+
+int thc_dgemm(thc_handle* h, int a_kmajor, int b_kmajor, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
+              int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc) {
+  if (!h || bad_ptr(A) || bad_ptr(B) || bad_ptr(C) || M <= 0 || N <= 0 || K <= 0) return THC_ERR_INVALID_ARG;
+  const int64_t lim = (int64_t)1 << 31;
+  if (M >= lim || N >= lim || K >= lim) return THC_ERR_OVERFLOW;
+  if (lda < (a_kmajor ? K : M) || ldb < (b_kmajor ? K : N) || ldc < N) return THC_ERR_INVALID_ARG;
+  DeviceGuard g(h->device);
+  if (!g.ok) return THC_ERR_CUDA;
+  Gemm gm(A, lda, a_kmajor ? 'K' : 'M', B, ldb, b_kmajor ? 'K' : 'N', C, ldc, M, N, K);
+  gm.ab(alpha, beta);
+  Ctx d{h}; d.dry = true; d.ar.dry = true;
+  d.gemm(gm);
+  Need need{0, d.splitk_need};
+  int st = ensure_workspace(h, std::max<i64>(h->need_bytes, need.total()));
+  if (st != THC_OK) return st;
+  Ctx c{h};
+  st = make_ctx(c, h, static_cast<char*>(h->ws), h->ws_bytes, need);
+  if (st != THC_OK) return st;
+  c.gemm(gm);
+  return c.status;
+}
+
+int thc_triple_product(thc_handle* h, int64_t nI, int64_t nPp, int64_t NPp, const double* E, const double* F,
+                       const double* G, double* H, int accumulate) {
+  if (!h || bad_ptr(E) || bad_ptr(F) || bad_ptr(G) || bad_ptr(H) || nI <= 0 || nPp <= 0 || NPp <= 0) return THC_ERR_INVALID_ARG;
+  if (nPp % thc::TP_PT != 0 || NPp % thc::TP_RT != 0) return THC_ERR_INVALID_ARG;
+  if (((reinterpret_cast<uintptr_t>(E) | reinterpret_cast<uintptr_t>(F) | reinterpret_cast<uintptr_t>(G) |
+        reinterpret_cast<uintptr_t>(H)) & 15) != 0)
+    return THC_ERR_INVALID_ARG;
+  DeviceGuard g(h->device);
+  if (!g.ok) return THC_ERR_CUDA;
+  Ctx c{h};
+  c.dry = false;
+  c.triple_product(E, F, G, H, nI, nPp, NPp, accumulate);
+  return c.status;
+}
+
+const char* thc_strerror(int status) {
+  switch (status) {
+    case THC_OK: return "ok";
+    case THC_ERR_INVALID_ARG: return "invalid argument (null or misaligned pointer, bad size)";
+    case THC_ERR_OVERFLOW: return "size overflow";
+    case THC_ERR_NO_MEMORY: return "workspace too small or device allocation failed";
+    case THC_ERR_CUDA: return "CUDA error (see thc_last_cuda_error)";
+    case THC_ERR_NO_DEVICE: return "no sm_100 CUDA device";
+    default: return "unknown status";
+  }
+}
+
+int thc_last_cuda_error(const thc_handle* h) { return h ? h->last_cuda : 0; }
+
+}  // extern "C"

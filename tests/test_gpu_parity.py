@@ -1,0 +1,115 @@
+"""Parity of the CUDA path (through the C ABI) against the dense CPU oracle, element by element.
+
+Tolerances (BASELINE.json north_star): max|R_gpu - R_ref| / max|R_ref| <= 1e-10 for the
+total AND for each of the six terms against that term's own maximum (the T2^2 terms are ~1e-6 of the total at the
+BASELINE Z scale, so a total-only check would not see them); |E_gpu - E_ref| <= 1e-9 E_h.
+"""
+import numpy as np
+import pytest
+
+from conftest import small_inputs, oracle_eval
+
+pytestmark = pytest.mark.gpu
+
+TERMS = ("s1", "s2", "s3", "s6", "s7", "s9")
+RTOL = 1e-10
+ETOL = 1e-9
+
+
+def _to_dev(x):
+    import torch
+    names = ("Xo", "Xv", "Z", "B_ov", "B_oo", "B_vv", "Y", "V", "eps")
+    return [torch.from_numpy(np.ascontiguousarray(getattr(x, n))).cuda() for n in names]
+
+
+def _relerr(got, ref):
+    scale = np.abs(ref).max()
+    if scale == 0.0:
+        return np.abs(got).max()
+    return np.abs(got - ref).max() / scale
+
+
+def _check_against(x, ref, **opts):
+    import torch
+    import paper_2111_11473_b200 as thc
+    h = thc.thc_setup(x.o, x.v, x.NL, x.NP, x.NX, **opts)
+    d = _to_dev(x)
+    res = h.thc_residual_terms(*d)
+    R2 = h.thc_residual(*d)
+    E = h.thc_energy(d[0], d[1], d[2], d[3])
+    torch.cuda.synchronize()
+    errs = {}
+    for k in TERMS + ("R", "xi_oo", "xi_vv"):
+        errs[k] = _relerr(res[k].cpu().numpy(), ref[k])
+    errs["R_direct"] = _relerr(R2.cpu().numpy(), ref["R"])
+    errs["E_abs"] = abs(E - ref["E"])
+    assert h.kernel_launches > 0
+    h.close()
+    bad = {k: e for k, e in errs.items() if e > (ETOL if k == "E_abs" else RTOL)}
+    assert not bad, f"parity failures {bad} (all: {errs})"
+    return errs
+
+
+def test_config0_per_term(oracle_cfg):
+    x, ref = oracle_cfg(0)
+    _check_against(x, ref)
+
+
+def test_config1_per_term(oracle_cfg):
+    x, ref = oracle_cfg(1)
+    _check_against(x, ref)
+
+
+@pytest.mark.parametrize("dims", [(3, 4, 6, 5, 7), (7, 13, 19, 37, 45), (6, 18, 10, 64, 96), (2, 35, 5, 33, 17)])
+def test_ragged_shapes_with_large_amplitudes(dims):
+    """Odd / non-multiple-of-tile extents (scalar load path, ragged tile tails); Z scaled up so that the
+    T2^2 terms are O(1) of the total."""
+    x = small_inputs(*dims, seed=11, zmul=30.0)
+    ref = oracle_eval(x)
+    _check_against(x, ref)
+
+
+@pytest.mark.parametrize("blocks", [dict(bL=1, bP7=1, bX=16, bI=1), dict(bL=5, bP7=7, bX=32, bI=9),
+                                    dict(bL=64, bP7=64, bX=64, bI=64)])
+def test_block_size_invariance(blocks):
+    """Results must not depend on the L / P / X / I blocking."""
+    x = small_inputs(6, 14, 21, 40, 52, seed=3, zmul=30.0)
+    ref = oracle_eval(x)
+    _check_against(x, ref, **blocks)
+
+
+def test_term_mask_and_zero_cases():
+    import torch
+    import paper_2111_11473_b200 as thc
+    x = small_inputs(4, 9, 8, 24, 30, seed=2, zmul=30.0)
+    ref = oracle_eval(x)
+    d = _to_dev(x)
+    for name, bit in thc.TERM_BITS.items():
+        h = thc.thc_setup(x.o, x.v, x.NL, x.NP, x.NX, term_mask=bit | (thc.TERM_BITS["s2"] if name == "s9" else 0))
+        res = h.thc_residual_terms(*d)
+        assert _relerr(res[name].cpu().numpy(), ref[name]) <= RTOL, name
+        h.close()
+    # Z = 0, B = 0  =>  R = 0 (north_star)
+    h = thc.thc_setup(x.o, x.v, x.NL, x.NP, x.NX)
+    z = [torch.zeros_like(t) for t in d]
+    R = h.thc_residual(d[0], d[1], z[2], z[3], z[4], z[5], d[6], d[7], d[8])
+    assert float(R.abs().max()) == 0.0
+    # Z = 0  =>  R = A A^T
+    R = h.thc_residual(d[0], d[1], z[2], d[3], d[4], d[5], d[6], d[7], d[8]).cpu().numpy()
+    A = np.einsum("iP,aP,Lia->PL", x.Xo, x.Xv, x.B_ov)
+    assert _relerr(R, A @ A.T) <= RTOL
+    h.close()
+
+
+def test_host_entry_matches_oracle(oracle_cfg):
+    import torch
+    import paper_2111_11473_b200 as thc
+    x, ref = oracle_cfg(0)
+    names = ("Xo", "Xv", "Z", "B_ov", "B_oo", "B_vv", "Y", "V", "eps")
+    host = [torch.from_numpy(np.ascontiguousarray(getattr(x, n))).pin_memory() for n in names]
+    R = torch.empty(x.NP, x.NP, dtype=torch.float64).pin_memory()
+    h = thc.thc_setup(x.o, x.v, x.NL, x.NP, x.NX)
+    E = h.thc_residual_host(*host, R)
+    assert _relerr(R.numpy(), ref["R"]) <= RTOL
+    assert abs(E - ref["E"]) <= ETOL
+    h.close()
