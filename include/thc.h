@@ -104,6 +104,10 @@ int thc_residual_terms(thc_handle* h, const double* Xo, const double* Xv, const 
 int thc_energy(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
                double* E_host);
 
+/* As thc_energy but asynchronous: E is written to the DEVICE address E_dev; no synchronisation. */
+int thc_energy_device(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
+                      double* E_dev);
+
 /* End-to-end entry with HOST buffers: copies every input host->device on the handle's stream, evaluates
  * R (and E if E_host != NULL), copies R device->host into R_host[NP][NP], synchronises.  The staging
  * buffers are part of the workspace (thc_workspace_bytes_host includes them).                       */
@@ -115,6 +119,14 @@ int thc_residual_host(thc_handle* h, const double* Xo, const double* Xv, const d
 int64_t thc_kernel_launches(const thc_handle* h);
 /* Algorithmic FP64 flop count of one residual evaluation for this shape (SURVEY.md 8(a) formulas). */
 double thc_algorithmic_flops(const thc_handle* h);
+
+/* Per-class kernel timing for roofline measurement.  After thc_profile_begin every kernel launch of a class
+ * whose bit is set in class_mask is bracketed by CUDA events on the handle's stream (bit 0: DMMA GEMM incl. its
+ * split-K reduction, bit 1: Alg.6 line 11 triple product, bit 2: Hadamard / reduction kernels).
+ * thc_profile_end synchronises the stream, returns the summed device time (milliseconds) and the number of timed
+ * launches per class, and switches the timing off again.  Not for use while the stream is being captured. */
+int thc_profile_begin(thc_handle* h, int class_mask);
+int thc_profile_end(thc_handle* h, double ms[3], int64_t counts[3]);
 
 /* Bare FP64 DMMA GEMM of the library (the kernel every GEMM chain uses), exposed for tests and roofline
  * measurement:  C[M][N] = alpha * sum_k A(m,k) B(n,k) + beta * C,  A(m,k) = A[m*lda+k] if a_kmajor else

@@ -21,7 +21,7 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
 # every symbol include/thc.h declares
 SYMBOLS = ("thc_setup", "thc_destroy", "thc_workspace_bytes", "thc_workspace_bytes_host", "thc_set_workspace",
            "thc_set_stream", "thc_get_blocks", "thc_residual", "thc_residual_terms", "thc_energy",
-           "thc_residual_host", "thc_kernel_launches", "thc_algorithmic_flops", "thc_dgemm",
+           "thc_energy_device", "thc_residual_host", "thc_profile_begin", "thc_profile_end", "thc_kernel_launches", "thc_algorithmic_flops", "thc_dgemm",
            "thc_triple_product", "thc_strerror", "thc_last_cuda_error")
 
 TERM_NAMES = ("s1", "s2", "s3", "s6", "s7", "s9")
@@ -79,6 +79,9 @@ def lib() -> ctypes.CDLL:
     L.thc_residual.argtypes = [VP] + [P] * 10
     L.thc_residual_terms.argtypes = [VP] + [P] * 10 + [ctypes.POINTER(P * 6), P, P]
     L.thc_energy.argtypes = [VP, P, P, P, P, ctypes.POINTER(D)]
+    L.thc_energy_device.argtypes = [VP, P, P, P, P, P]
+    L.thc_profile_begin.argtypes = [VP, ctypes.c_int]
+    L.thc_profile_end.argtypes = [VP, ctypes.POINTER(D * 3), ctypes.POINTER(I64 * 3)]
     L.thc_residual_host.argtypes = [VP] + [P] * 10 + [ctypes.POINTER(D)]
     L.thc_kernel_launches.argtypes = [VP]
     L.thc_kernel_launches.restype = I64
@@ -214,6 +217,26 @@ class Thc:
         _check(lib().thc_energy(self._h, _dev_ptr(Xo, "Xo", o * NP), _dev_ptr(Xv, "Xv", v * NP),
                                 _dev_ptr(Z, "Z", NP * NP), _dev_ptr(B_ov, "B_ov", NL * o * v), ctypes.byref(E)), self._h)
         return E.value
+
+    def thc_energy_device(self, Xo, Xv, Z, B_ov, out=None):
+        """E as a 1-element device tensor (asynchronous on torch's current stream)."""
+        import torch
+        self._prepare(self.workspace_bytes)
+        o, v, NL, NP = self.o, self.v, self.NL, self.NP
+        E = out if out is not None else torch.empty(1, dtype=torch.float64, device=self._device)
+        _check(lib().thc_energy_device(self._h, _dev_ptr(Xo, "Xo", o * NP), _dev_ptr(Xv, "Xv", v * NP),
+                                       _dev_ptr(Z, "Z", NP * NP), _dev_ptr(B_ov, "B_ov", NL * o * v),
+                                       _dev_ptr(E, "E", 1)), self._h)
+        return E
+
+    def thc_profile_begin(self, class_mask=7):
+        _check(lib().thc_profile_begin(self._h, int(class_mask)), self._h)
+
+    def thc_profile_end(self):
+        """{class: (milliseconds, launches)} for classes gemm / triple / ew; synchronises the stream."""
+        ms, cnt = (ctypes.c_double * 3)(), (ctypes.c_int64 * 3)()
+        _check(lib().thc_profile_end(self._h, ctypes.byref(ms), ctypes.byref(cnt)), self._h)
+        return {k: (ms[i], cnt[i]) for i, k in enumerate(("gemm", "triple", "ew"))}
 
     def thc_residual_host(self, Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps, R_host, want_energy=True):
         """End-to-end entry: HOST tensors in, R written into the host tensor R_host, returns E (or None)."""

@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <algorithm>
+#include <vector>
 #include "../../include/thc.h"
 #include "thc_gemm.cuh"
 #include "thc_kernels.cuh"
@@ -22,6 +23,12 @@ struct thc_handle {
   int64_t launches;
   int last_cuda;
   bool smem_configured;
+  // per-class kernel timing (thc_profile_begin / thc_profile_end): CUDA events recorded on `stream` around every
+  // launch of a class whose bit is set in prof_mask
+  int prof_mask;
+  std::vector<cudaEvent_t> prof_events;     // pool; pairs (start, stop)
+  std::vector<int> prof_class;              // class of pair k
+  size_t prof_used;                         // pairs in use
 };
 
 namespace thc {
@@ -101,6 +108,24 @@ struct Ctx {
     if (e != cudaSuccess && status == THC_OK) { status = THC_ERR_CUDA; h->last_cuda = (int)e; }
   }
   void launched() { h->launches++; check(cudaPeekAtLastError()); }
+  // kernel classes for thc_profile_*: 0 = DMMA GEMM (+ its split-K reduce), 1 = Alg.6 line 11, 2 = Hadamard / reduction
+  void prof_start(int cls) {
+    if (!(h->prof_mask & (1 << cls))) return;
+    if (h->prof_used * 2 + 2 > h->prof_events.size()) {
+      cudaEvent_t a, b;
+      if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { check(cudaGetLastError()); return; }
+      h->prof_events.push_back(a); h->prof_events.push_back(b);
+      h->prof_class.push_back(cls);
+    }
+    h->prof_class[h->prof_used] = cls;
+    cudaEventRecord(h->prof_events[h->prof_used * 2], h->stream);
+  }
+  void prof_stop(int cls) {
+    if (!(h->prof_mask & (1 << cls))) return;
+    if (h->prof_used * 2 + 2 > h->prof_events.size()) return;
+    cudaEventRecord(h->prof_events[h->prof_used * 2 + 1], h->stream);
+    h->prof_used++;
+  }
   int ew_blocks(i64 n, int per = 256) const { return (int)std::max<i64>(1, std::min<i64>((n + per - 1) / per, (i64)h->sms * 16)); }
 
   // ---- GEMM ----------------------------------------------------------------------------------------------------
@@ -139,6 +164,7 @@ struct Ctx {
     if (zdim > 65535) { status = THC_ERR_INVALID_ARG; return; }
     dim3 grid((unsigned)tiles_mn, 1, (unsigned)zdim);
     cudaError_t e;
+    prof_start(0);
     const int sel = (g.akm ? 4 : 0) | (g.bkm ? 2 : 0) | (al16 ? 1 : 0);
     switch (sel) {
       case 7: e = launch_gemm_variant<true, true, true>(big, grid, h->stream, p); break;
@@ -161,21 +187,26 @@ struct Ctx {
       reduce_splits_kernel<<<ew_blocks(per), 256, 0, h->stream>>>(r);
       launched();
     }
+    prof_stop(0);
   }
 
   // ---- element-wise / reduction launches -------------------------------------------------------------------------
 #define THC_EW(kernel, n, ...)                                          \
   do {                                                                  \
     if (dry || !ok()) return;                                           \
+    prof_start(2);                                                      \
     kernel<<<ew_blocks(n), 256, 0, h->stream>>>(__VA_ARGS__);           \
     launched();                                                         \
+    prof_stop(2);                                                       \
   } while (0)
 
   void transpose(const double* in, double* out, i64 rows, i64 cols) {
     if (dry || !ok()) return;
     dim3 grid((unsigned)((cols + 31) / 32), (unsigned)((rows + 31) / 32)), blk(32, 8);
+    prof_start(2);
     transpose_kernel<<<grid, blk, 0, h->stream>>>(in, out, (int)rows, (int)cols);
     launched();
+    prof_stop(2);
   }
   void fill(double* x, i64 n, double val) { THC_EW(fill_kernel, n, x, n, val); }
   void hadamard(const double* a, const double* b, double* out, i64 n) { THC_EW(hadamard_kernel, n, a, b, out, n); }
@@ -207,8 +238,10 @@ struct Ctx {
   void symmetrize(const double* P, double* out, i64 n, double scale) {
     if (dry || !ok()) return;
     dim3 grid((unsigned)((n + 31) / 32), (unsigned)((n + 31) / 32)), blk(32, 8);
+    prof_start(2);
     symmetrize_kernel<<<grid, blk, 0, h->stream>>>(P, out, (int)n, scale);
     launched();
+    prof_stop(2);
   }
   void fock(const double* eps, const double* xi_oo, const double* xi_vv, double* FooT, double* Fvv, i64 o, i64 v) {
     THC_EW(fock_kernel, o * o + v * v, eps, xi_oo, xi_vv, FooT, Fvv, (int)o, (int)v);
@@ -220,21 +253,27 @@ struct Ctx {
   int dot_blocks(i64 n) const { return ew_blocks(n, 1024); }
   void dot_partial(const double* a, const double* b, i64 n, double* partial) {
     if (dry || !ok()) return;
+    prof_start(2);
     dot_partial_kernel<<<dot_blocks(n), 256, 0, h->stream>>>(a, b, n, partial);
     launched();
+    prof_stop(2);
   }
   i64 zee_blocks(i64 NP, i64 nl) const { i64 t = (NP + 31) / 32; return t * t * nl; }
   void zee_partial(const double* Z, const double* E, i64 NP, i64 nl, double* partial) {
     if (dry || !ok()) return;
     unsigned t = (unsigned)((NP + 31) / 32);
     dim3 grid(t, t, (unsigned)nl), blk(32, 8);
+    prof_start(2);
     zee_partial_kernel<<<grid, blk, 0, h->stream>>>(Z, E, (int)NP, partial);
     launched();
+    prof_stop(2);
   }
   void final_sum(const double* pa, i64 na, double ca, const double* pb, i64 nb, double cb, double* out, int accumulate) {
     if (dry || !ok()) return;
+    prof_start(2);
     final_sum_kernel<<<1, 1024, 0, h->stream>>>(pa, na, ca, pb, nb, cb, out, accumulate);
     launched();
+    prof_stop(2);
   }
   void triple_product(const double* E, const double* F, const double* G, double* H, i64 nI, i64 nPp, i64 NPp, int accumulate) {
     if (dry || !ok()) return;
@@ -247,8 +286,10 @@ struct Ctx {
     p.nI = (int)nI; p.nPp = (int)nPp; p.NPp = (int)NPp; p.accumulate = accumulate;
     i64 nrb = NPp / TP_RT;
     dim3 grid((unsigned)(nrb * (nrb + 1)), (unsigned)(nPp / TP_PT));
+    prof_start(1);
     triple_product_kernel<<<grid, 256, TP_SMEM_BYTES, h->stream>>>(p);
     launched();
+    prof_stop(1);
   }
 };
 

@@ -369,17 +369,19 @@ int run_residual(thc_handle* h, char* base, i64 bytes, const Inputs& in, const O
   return c.status;
 }
 int run_energy(thc_handle* h, char* base, i64 bytes, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
-               double* E_host) {
+               double* E_host, double* E_dev) {
   Need need = dry_energy(h);
   Ctx c{h};
   int st = make_ctx(c, h, base, bytes, need);
   if (st != THC_OK) return st;
   double* e = c.ar.alloc(1);
-  plan_energy(c, Xo, Xv, Z, B_ov, e);
+  plan_energy(c, Xo, Xv, Z, B_ov, E_dev ? E_dev : e);
   if (c.ar.overflow) return THC_ERR_NO_MEMORY;
   if (c.status != THC_OK) return c.status;
-  c.check(cudaMemcpyAsync(E_host, e, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
-  c.check(cudaStreamSynchronize(h->stream));
+  if (E_host) {
+    c.check(cudaMemcpyAsync(E_host, E_dev ? E_dev : e, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    c.check(cudaStreamSynchronize(h->stream));
+  }
   return c.status;
 }
 
@@ -418,6 +420,7 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
   h->device = dev; h->sms = prop.multiProcessorCount;
   h->stream = nullptr; h->ws = nullptr; h->ws_bytes = 0; h->ws_owned = false;
   h->launches = 0; h->last_cuda = 0; h->smem_configured = false;
+  h->prof_mask = 0; h->prof_used = 0;
 
   // block sizes: defaults, then shrink until the plan fits the cap
   h->bL = std::min<int64_t>(NL, (opt && opt->bL) ? opt->bL : 32);
@@ -450,10 +453,11 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
 
 int thc_destroy(thc_handle* h) {
   if (!h) return THC_ERR_INVALID_ARG;
-  if (h->ws && h->ws_owned) {
+  if ((h->ws && h->ws_owned) || !h->prof_events.empty()) {
     DeviceGuard g(h->device);
     cudaStreamSynchronize(h->stream);
-    cudaFree(h->ws);
+    if (h->ws && h->ws_owned) cudaFree(h->ws);
+    for (cudaEvent_t e : h->prof_events) cudaEventDestroy(e);
   }
   delete h;
   return THC_OK;
@@ -519,7 +523,42 @@ int thc_energy(thc_handle* h, const double* Xo, const double* Xv, const double* 
   if (!g.ok) return THC_ERR_CUDA;
   int st = ensure_workspace(h, h->need_bytes);
   if (st != THC_OK) return st;
-  return run_energy(h, static_cast<char*>(h->ws), h->ws_bytes, Xo, Xv, Z, B_ov, E_host);
+  return run_energy(h, static_cast<char*>(h->ws), h->ws_bytes, Xo, Xv, Z, B_ov, E_host, nullptr);
+}
+
+int thc_energy_device(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov, double* E_dev) {
+  if (!h || bad_ptr(Xo) || bad_ptr(Xv) || bad_ptr(Z) || bad_ptr(B_ov) || bad_ptr(E_dev)) return THC_ERR_INVALID_ARG;
+  DeviceGuard g(h->device);
+  if (!g.ok) return THC_ERR_CUDA;
+  int st = ensure_workspace(h, h->need_bytes);
+  if (st != THC_OK) return st;
+  return run_energy(h, static_cast<char*>(h->ws), h->ws_bytes, Xo, Xv, Z, B_ov, nullptr, E_dev);
+}
+
+int thc_profile_begin(thc_handle* h, int class_mask) {
+  if (!h || class_mask < 0 || class_mask > 7) return THC_ERR_INVALID_ARG;
+  h->prof_mask = class_mask;
+  h->prof_used = 0;
+  return THC_OK;
+}
+
+int thc_profile_end(thc_handle* h, double ms[3], int64_t counts[3]) {
+  if (!h || !ms || !counts) return THC_ERR_INVALID_ARG;
+  DeviceGuard g(h->device);
+  if (!g.ok) return THC_ERR_CUDA;
+  for (int k = 0; k < 3; k++) { ms[k] = 0.0; counts[k] = 0; }
+  cudaError_t e = cudaStreamSynchronize(h->stream);
+  if (e != cudaSuccess) { h->last_cuda = (int)e; return THC_ERR_CUDA; }
+  for (size_t k = 0; k < h->prof_used; k++) {
+    float t = 0.f;
+    e = cudaEventElapsedTime(&t, h->prof_events[2 * k], h->prof_events[2 * k + 1]);
+    if (e != cudaSuccess) { h->last_cuda = (int)e; return THC_ERR_CUDA; }
+    ms[h->prof_class[k]] += (double)t;
+    counts[h->prof_class[k]]++;
+  }
+  h->prof_mask = 0;
+  h->prof_used = 0;
+  return THC_OK;
 }
 
 int thc_residual_host(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
@@ -555,7 +594,7 @@ int thc_residual_host(thc_handle* h, const double* Xo, const double* Xv, const d
   cudaError_t e = cudaMemcpyAsync(R_host, Rd, (size_t)h->NP * h->NP * 8, cudaMemcpyDeviceToHost, h->stream);
   if (e != cudaSuccess) { h->last_cuda = (int)e; return THC_ERR_CUDA; }
   if (E_host) {
-    st = run_energy(h, p, rest, dev[0], dev[1], dev[2], dev[3], E_host);   // synchronises
+    st = run_energy(h, p, rest, dev[0], dev[1], dev[2], dev[3], E_host, nullptr);   // synchronises
     if (st != THC_OK) return st;
   }
   e = cudaStreamSynchronize(h->stream);
