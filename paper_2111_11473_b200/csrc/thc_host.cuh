@@ -4,11 +4,14 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <stdio.h>
 #include <algorithm>
+#include <string>
 #include <vector>
 #include "../../include/thc.h"
 #include "thc_gemm.cuh"
 #include "thc_kernels.cuh"
+#include "thc_triple.cuh"
 
 struct thc_handle {
   int64_t o, v, NL, NP, NX;
@@ -23,11 +26,17 @@ struct thc_handle {
   int64_t launches;
   int last_cuda;
   bool smem_configured;
+  // Alg.6 line 11: work-item lists (device memory owned by the handle), one per (nPp, NPp) shape seen
+  struct TripleList { int64_t nPp, NPp; thc::TripleItem* dev; int n; };
+  std::vector<TripleList> tp_lists;
+  void* encode_tiled;                // cuTensorMapEncodeTiled, resolved through the runtime (no -lcuda link)
   // per-class kernel timing (thc_profile_begin / thc_profile_end): CUDA events recorded on `stream` around every
   // launch of a class whose bit is set in prof_mask
   int prof_mask;
   std::vector<cudaEvent_t> prof_events;     // pool; pairs (start, stop)
   std::vector<int> prof_class;              // class of pair k
+  std::vector<std::string> prof_desc;       // what pair k timed (printed by thc_profile_end when THC_TRACE is set)
+  std::vector<double> prof_flops;
   size_t prof_used;                         // pairs in use
 };
 
@@ -109,15 +118,19 @@ struct Ctx {
   }
   void launched() { h->launches++; check(cudaPeekAtLastError()); }
   // kernel classes for thc_profile_*: 0 = DMMA GEMM (+ its split-K reduce), 1 = Alg.6 line 11, 2 = Hadamard / reduction
-  void prof_start(int cls) {
+  void prof_start(int cls, const char* desc = "", double flops = 0.0) {
     if (!(h->prof_mask & (1 << cls))) return;
     if (h->prof_used * 2 + 2 > h->prof_events.size()) {
       cudaEvent_t a, b;
       if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { check(cudaGetLastError()); return; }
       h->prof_events.push_back(a); h->prof_events.push_back(b);
       h->prof_class.push_back(cls);
+      h->prof_desc.emplace_back();
+      h->prof_flops.push_back(0.0);
     }
     h->prof_class[h->prof_used] = cls;
+    h->prof_desc[h->prof_used] = desc;
+    h->prof_flops[h->prof_used] = flops;
     cudaEventRecord(h->prof_events[h->prof_used * 2], h->stream);
   }
   void prof_stop(int cls) {
@@ -164,7 +177,11 @@ struct Ctx {
     if (zdim > 65535) { status = THC_ERR_INVALID_ARG; return; }
     dim3 grid((unsigned)tiles_mn, 1, (unsigned)zdim);
     cudaError_t e;
-    prof_start(0);
+    char desc[160];
+    if (h->prof_mask & 1)
+      snprintf(desc, sizeof desc, "gemm %s M=%d N=%d K=%d batch=%d kbatch=%d splits=%d %c%c%s", big ? "big" : "small", g.M, g.N, g.K,
+               g.nbatch, g.nkb, splits, g.akm ? 'K' : 'M', g.bkm ? 'K' : 'N', al16 ? "" : " unaligned");
+    prof_start(0, desc, 2.0 * g.M * g.N * (double)g.K * g.nbatch * g.nkb);
     const int sel = (g.akm ? 4 : 0) | (g.bkm ? 2 : 0) | (al16 ? 1 : 0);
     switch (sel) {
       case 7: e = launch_gemm_variant<true, true, true>(big, grid, h->stream, p); break;
@@ -194,7 +211,7 @@ struct Ctx {
 #define THC_EW(kernel, n, ...)                                          \
   do {                                                                  \
     if (dry || !ok()) return;                                           \
-    prof_start(2);                                                      \
+    prof_start(2, #kernel, (double)(n));                                                    \
     kernel<<<ew_blocks(n), 256, 0, h->stream>>>(__VA_ARGS__);           \
     launched();                                                         \
     prof_stop(2);                                                       \
@@ -275,19 +292,65 @@ struct Ctx {
     launched();
     prof_stop(2);
   }
+  // TMA descriptor over a [d2][d1][d0] FP64 array (d0 contiguous), box 16 x 16 x 1, 128-byte swizzle.
+  bool make_map3(CUtensorMap* m, const double* base, i64 d0, i64 d1, i64 d2) {
+    typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    if (!h->encode_tiled) {
+      void* fn = nullptr;
+      cudaDriverEntryPointQueryResult q;
+      if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn) {
+        check(cudaErrorNotSupported);
+        return false;
+      }
+      h->encode_tiled = fn;
+    }
+    const cuuint64_t dims[3] = {(cuuint64_t)d0, (cuuint64_t)d1, (cuuint64_t)d2};
+    const cuuint64_t strides[2] = {(cuuint64_t)d0 * 8, (cuuint64_t)d0 * (cuuint64_t)d1 * 8};
+    const cuuint32_t box[3] = {16, 16, 1}, es[3] = {1, 1, 1};
+    CUresult r = reinterpret_cast<EncodeFn>(h->encode_tiled)(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<double*>(base), dims,
+                                                             strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                                             CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { check(cudaErrorInvalidValue); return false; }
+    return true;
+  }
+  // Work items of Alg.6 line 11 in an L2-friendly order: groups of 8 p-tiles x 6 q-tiles x 3 r-tiles run at the same time.
+  const thc_handle::TripleList* triple_items(i64 nPp, i64 NPp) {
+    for (const auto& l : h->tp_lists) if (l.nPp == nPp && l.NPp == NPp) return &l;
+    std::vector<TripleItem> items;
+    const int npt = (int)(nPp / TP_PT), nqb = (int)(NPp / TP_QT), nrb = (int)(NPp / TP_RT);
+    for (int rb0 = 0; rb0 < nrb; rb0 += 3)
+      for (int qb0 = 0; qb0 < nqb && qb0 <= 2 * std::min(rb0 + 2, nrb - 1) + 1; qb0 += 6)
+        for (int pt0 = 0; pt0 < npt; pt0 += 8)
+          for (int pt = pt0; pt < std::min(pt0 + 8, npt); pt++)
+            for (int rb = rb0; rb < std::min(rb0 + 3, nrb); rb++)
+              for (int qb = qb0; qb < std::min(qb0 + 6, nqb); qb++)
+                if (qb <= 2 * rb + 1) items.push_back(TripleItem{pt * TP_PT, qb * TP_QT, rb * TP_RT, (qb >> 1) == rb ? 1 : 0});
+    thc_handle::TripleList l{nPp, NPp, nullptr, (int)items.size()};
+    if (cudaMalloc(&l.dev, items.size() * sizeof(TripleItem)) != cudaSuccess) { check(cudaGetLastError()); return nullptr; }
+    // pageable source: the runtime stages the data before returning, so `items` may die at the end of this scope
+    check(cudaMemcpyAsync(l.dev, items.data(), items.size() * sizeof(TripleItem), cudaMemcpyHostToDevice, h->stream));
+    check(cudaStreamSynchronize(h->stream));
+    h->tp_lists.push_back(l);
+    return &h->tp_lists.back();
+  }
   void triple_product(const double* E, const double* F, const double* G, double* H, i64 nI, i64 nPp, i64 NPp, int accumulate) {
     if (dry || !ok()) return;
     if (!h->smem_configured) {
       check(cudaFuncSetAttribute(triple_product_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TP_SMEM_BYTES));
       h->smem_configured = true;
     }
+    const thc_handle::TripleList* list = triple_items(nPp, NPp);
+    CUtensorMap mE, mF, mG;
+    if (!list || !make_map3(&mE, E, NPp, nPp, nI) || !make_map3(&mF, F, NPp, nPp, nI) || !make_map3(&mG, G, NPp, NPp, nI)) return;
     TripleParams p;
-    p.E = E; p.F = F; p.G = G; p.H = H;
+    p.H = H; p.items = list->dev; p.n_items = list->n;
     p.nI = (int)nI; p.nPp = (int)nPp; p.NPp = (int)NPp; p.accumulate = accumulate;
-    i64 nrb = NPp / TP_RT;
-    dim3 grid((unsigned)(nrb * (nrb + 1)), (unsigned)(nPp / TP_PT));
-    prof_start(1);
-    triple_product_kernel<<<grid, 256, TP_SMEM_BYTES, h->stream>>>(p);
+    const int grid = std::min(list->n, h->sms);
+    if (((i64)(list->n + grid - 1) / grid) * nI >= ((i64)1 << 31)) { status = THC_ERR_OVERFLOW; return; }
+    prof_start(1, "triple_product", 5.0 * nI * nPp * (double)NPp * NPp);
+    triple_product_kernel<<<grid, TP_THREADS, TP_SMEM_BYTES, h->stream>>>(mE, mF, mG, p);
     launched();
     prof_stop(1);
   }

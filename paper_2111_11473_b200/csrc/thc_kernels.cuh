@@ -238,190 +238,4 @@ __global__ void final_sum_kernel(const double* __restrict__ pa, i64 na, double c
   if (threadIdx.x == 0) out[0] = accumulate ? out[0] + s : s;
 }
 
-// ------------------------------------------------------------------------------------------------------------------
-// Alg.6 line 11 (l.714):  H[p][q][r] += sum_I (E_I[p][q] F_I[p][r] + E_I[p][r] F_I[p][q]) G_I[q][r]
-//
-// The bracket s_I[p](q,r) is symmetric in (q,r), so a CTA that owns the (p, q-tile, r-tile) block with the q-tile
-// strictly below the r-tile also owns the mirrored block (p, r-tile, q-tile): s is formed once (2 FP64 instr) and
-// used twice (2 FMA) -> 2 instead of 3 FP64 instructions per (p,q,r,I).  CTAs whose q-tile lies inside their r-tile
-// (the diagonal) do the plain 3-instruction update for every (q,r) of the block.
-//
-// CTA = 256 threads = 8 warps as (2 p) x (2 q) x (2 r); lane = (lp 2) x (lq 4) x (lr 4); thread tile (4 p, 2 q, 4 r)
-// => warp tile 8 x 8 x 16, CTA tile 16 x 16 x 32, 64 accumulators per thread.  Per I the CTA reads six operand
-// tiles from shared memory (E,F over (p,q); E,F over (p,r); G over (q,r); G over (r,q)), staged by cp.async in
-// chunks of TP_IC grid points, TP_STAGES deep.  Row pitches (18 / 34 doubles) make every 16-byte fragment load
-// conflict-free: see DESIGN.md section 6.
-constexpr int TP_PT = 16, TP_QT = 16, TP_RT = 32, TP_IC = 2, TP_STAGES = 3;
-constexpr int TP_PQ_PITCH = 18, TP_PR_PITCH = 34;
-constexpr int TP_OFF_EPQ = 0;
-constexpr int TP_OFF_FPQ = TP_OFF_EPQ + TP_PT * TP_PQ_PITCH;
-constexpr int TP_OFF_EPR = TP_OFF_FPQ + TP_PT * TP_PQ_PITCH;
-constexpr int TP_OFF_FPR = TP_OFF_EPR + TP_PT * TP_PR_PITCH;
-constexpr int TP_OFF_GQR = TP_OFF_FPR + TP_PT * TP_PR_PITCH;
-constexpr int TP_OFF_GRQ = TP_OFF_GQR + TP_QT * TP_PR_PITCH;
-constexpr int TP_PER_I = TP_OFF_GRQ + TP_RT * TP_PQ_PITCH;       // doubles per grid point
-constexpr int TP_STAGE = TP_PER_I * TP_IC;
-constexpr int TP_SMEM_BYTES = TP_STAGE * TP_STAGES * 8;
-
-struct TripleParams {
-  const double* E; const double* F; const double* G; double* H;
-  int nI, nPp, NPp;        // padded extents: nPp % 16 == 0, NPp % 32 == 0
-  int accumulate;
-};
-
-__device__ __forceinline__ void tp_copy_rows(double* s, int pitch, const double* g, i64 ld, int rows, int cols, int tid) {
-  // rows x cols doubles (cols % 2 == 0), 16-byte chunks
-  int cpr = cols / 2, total = rows * cpr;
-  for (int c = tid; c < total; c += 256) {
-    int r = c / cpr, cc = c % cpr;
-    cp_async16(s + r * pitch + cc * 2, g + (i64)r * ld + cc * 2, 16);
-  }
-}
-
-__global__ void __launch_bounds__(256) triple_product_kernel(const TripleParams p) {
-  extern __shared__ __align__(16) double smem[];
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int wp = warp >> 2, wq = (warp >> 1) & 1, wr = warp & 1;
-  const int lp = lane >> 4, lq = (lane >> 2) & 3, lr = lane & 3;
-  // tile coordinates: blockIdx.x enumerates (qb, rb) with qb/2 <= rb; blockIdx.y = p tile
-  const int nrb = p.NPp / TP_RT;
-  int rb = 0, qb = 0;
-  {
-    // pairs are ordered rb-major: rb = 0 has qb in [0, 2), rb = 1 has [0, 4), ...  -> offset(rb) = rb (rb + 1)
-    int x = blockIdx.x;
-    rb = (int)((sqrtf(4.0f * x + 1.0f) - 1.0f) * 0.5f);
-    while (rb * (rb + 1) > x) rb--;
-    while ((rb + 1) * (rb + 2) <= x) rb++;
-    qb = x - rb * (rb + 1);
-  }
-  (void)nrb;
-  const bool diag = (qb >> 1) == rb;
-  const int p0 = blockIdx.y * TP_PT, q0 = qb * TP_QT, r0 = rb * TP_RT;
-  const i64 ldE = p.NPp, sEI = (i64)p.nPp * p.NPp;      // E[I][p][q]
-  const i64 ldG = p.NPp, sGI = (i64)p.NPp * p.NPp;      // G[I][q][r]
-
-  // thread's indices inside the CTA tile
-  const int tp0 = wp * 8 + lp * 4;                      // 4 consecutive p
-  const int tq0 = wq * 8 + lq * 2;                      // 2 consecutive q
-  const int trA = wr * 16 + lr * 2, trB = trA + 8;      // r pairs {trA, trA+1}, {trB, trB+1}
-
-  double hqr[4][2][4], hrq[4][2][4];
-#pragma unroll
-  for (int a = 0; a < 4; a++)
-#pragma unroll
-    for (int b = 0; b < 2; b++)
-#pragma unroll
-      for (int c = 0; c < 4; c++) hqr[a][b][c] = hrq[a][b][c] = 0.0;
-
-  const int nchunks = (p.nI + TP_IC - 1) / TP_IC;
-  auto issue = [&](int ch) {
-    if (ch < nchunks) {
-      double* st = smem + (ch % TP_STAGES) * TP_STAGE;
-      for (int ii = 0; ii < TP_IC; ii++) {
-        int I = ch * TP_IC + ii;
-        if (I >= p.nI) break;
-        double* s = st + ii * TP_PER_I;
-        const double* Eg = p.E + (i64)I * sEI + (i64)p0 * ldE;
-        const double* Fg = p.F + (i64)I * sEI + (i64)p0 * ldE;
-        const double* Gg = p.G + (i64)I * sGI;
-        tp_copy_rows(s + TP_OFF_EPQ, TP_PQ_PITCH, Eg + q0, ldE, TP_PT, TP_QT, tid);
-        tp_copy_rows(s + TP_OFF_FPQ, TP_PQ_PITCH, Fg + q0, ldE, TP_PT, TP_QT, tid);
-        tp_copy_rows(s + TP_OFF_EPR, TP_PR_PITCH, Eg + r0, ldE, TP_PT, TP_RT, tid);
-        tp_copy_rows(s + TP_OFF_FPR, TP_PR_PITCH, Fg + r0, ldE, TP_PT, TP_RT, tid);
-        tp_copy_rows(s + TP_OFF_GQR, TP_PR_PITCH, Gg + (i64)q0 * ldG + r0, ldG, TP_QT, TP_RT, tid);
-        if (!diag) tp_copy_rows(s + TP_OFF_GRQ, TP_PQ_PITCH, Gg + (i64)r0 * ldG + q0, ldG, TP_RT, TP_QT, tid);
-      }
-    }
-    cp_async_commit();
-  };
-#pragma unroll
-  for (int s = 0; s < TP_STAGES - 1; s++) issue(s);
-
-  for (int ch = 0; ch < nchunks; ch++) {
-    cp_async_wait<TP_STAGES - 2>();
-    __syncthreads();
-    issue(ch + TP_STAGES - 1);
-    const double* st = smem + (ch % TP_STAGES) * TP_STAGE;
-    const int ni = min(TP_IC, p.nI - ch * TP_IC);
-    for (int ii = 0; ii < ni; ii++) {
-      const double* s = st + ii * TP_PER_I;
-      double epq[4][2], fpq[4][2], epr[4][4], fpr[4][4], gqr[2][4];
-#pragma unroll
-      for (int a = 0; a < 4; a++) {
-        double2 x = *reinterpret_cast<const double2*>(s + TP_OFF_EPQ + (tp0 + a) * TP_PQ_PITCH + tq0);
-        double2 y = *reinterpret_cast<const double2*>(s + TP_OFF_FPQ + (tp0 + a) * TP_PQ_PITCH + tq0);
-        epq[a][0] = x.x; epq[a][1] = x.y; fpq[a][0] = y.x; fpq[a][1] = y.y;
-        double2 e0 = *reinterpret_cast<const double2*>(s + TP_OFF_EPR + (tp0 + a) * TP_PR_PITCH + trA);
-        double2 e1 = *reinterpret_cast<const double2*>(s + TP_OFF_EPR + (tp0 + a) * TP_PR_PITCH + trB);
-        double2 f0 = *reinterpret_cast<const double2*>(s + TP_OFF_FPR + (tp0 + a) * TP_PR_PITCH + trA);
-        double2 f1 = *reinterpret_cast<const double2*>(s + TP_OFF_FPR + (tp0 + a) * TP_PR_PITCH + trB);
-        epr[a][0] = e0.x; epr[a][1] = e0.y; epr[a][2] = e1.x; epr[a][3] = e1.y;
-        fpr[a][0] = f0.x; fpr[a][1] = f0.y; fpr[a][2] = f1.x; fpr[a][3] = f1.y;
-      }
-#pragma unroll
-      for (int b = 0; b < 2; b++) {
-        double2 g0 = *reinterpret_cast<const double2*>(s + TP_OFF_GQR + (tq0 + b) * TP_PR_PITCH + trA);
-        double2 g1 = *reinterpret_cast<const double2*>(s + TP_OFF_GQR + (tq0 + b) * TP_PR_PITCH + trB);
-        gqr[b][0] = g0.x; gqr[b][1] = g0.y; gqr[b][2] = g1.x; gqr[b][3] = g1.y;
-      }
-      if (!diag) {
-        double grq[4][2];
-#pragma unroll
-        for (int c = 0; c < 4; c++) {
-          int r = (c < 2) ? trA + c : trB + (c - 2);
-          double2 gg = *reinterpret_cast<const double2*>(s + TP_OFF_GRQ + r * TP_PQ_PITCH + tq0);
-          grq[c][0] = gg.x; grq[c][1] = gg.y;
-        }
-#pragma unroll
-        for (int a = 0; a < 4; a++)
-#pragma unroll
-          for (int b = 0; b < 2; b++)
-#pragma unroll
-            for (int c = 0; c < 4; c++) {
-              double sv = fma(epr[a][c], fpq[a][b], epq[a][b] * fpr[a][c]);
-              hqr[a][b][c] = fma(sv, gqr[b][c], hqr[a][b][c]);
-              hrq[a][b][c] = fma(sv, grq[c][b], hrq[a][b][c]);
-            }
-      } else {
-#pragma unroll
-        for (int a = 0; a < 4; a++)
-#pragma unroll
-          for (int b = 0; b < 2; b++)
-#pragma unroll
-            for (int c = 0; c < 4; c++) {
-              double sv = fma(epr[a][c], fpq[a][b], epq[a][b] * fpr[a][c]);
-              hqr[a][b][c] = fma(sv, gqr[b][c], hqr[a][b][c]);
-            }
-      }
-    }
-  }
-  cp_async_wait<0>();
-
-  // write back: H[p][q][r]
-  const i64 sHp = (i64)p.NPp * p.NPp;
-#pragma unroll
-  for (int a = 0; a < 4; a++) {
-    double* Hp = p.H + (i64)(p0 + tp0 + a) * sHp;
-#pragma unroll
-    for (int b = 0; b < 2; b++) {
-      double* row = Hp + (i64)(q0 + tq0 + b) * p.NPp + r0;
-      double2* d0 = reinterpret_cast<double2*>(row + trA);
-      double2* d1 = reinterpret_cast<double2*>(row + trB);
-      double2 v0 = make_double2(hqr[a][b][0], hqr[a][b][1]), v1 = make_double2(hqr[a][b][2], hqr[a][b][3]);
-      if (p.accumulate) { double2 o0 = *d0, o1 = *d1; v0.x += o0.x; v0.y += o0.y; v1.x += o1.x; v1.y += o1.y; }
-      *d0 = v0; *d1 = v1;
-    }
-    if (!diag) {
-#pragma unroll
-      for (int c = 0; c < 4; c++) {
-        int r = (c < 2) ? trA + c : trB + (c - 2);
-        double2* d = reinterpret_cast<double2*>(Hp + (i64)(r0 + r) * p.NPp + q0 + tq0);
-        double2 vv = make_double2(hrq[a][0][c], hrq[a][1][c]);
-        if (p.accumulate) { double2 o = *d; vv.x += o.x; vv.y += o.y; }
-        *d = vv;
-      }
-    }
-  }
-}
-
 }  // namespace thc

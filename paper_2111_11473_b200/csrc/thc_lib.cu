@@ -10,6 +10,7 @@
 //   * Alg.6 line 11 (l.714) runs on the FP64 FMA pipe (triple_product_kernel).
 // Notation: P,Q,R amplitude grid (paper W,X,Y,Z), I,J ERI grid, L Cholesky index (paper A); see DESIGN.md.
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include "thc_host.cuh"
@@ -420,7 +421,7 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
   h->device = dev; h->sms = prop.multiProcessorCount;
   h->stream = nullptr; h->ws = nullptr; h->ws_bytes = 0; h->ws_owned = false;
   h->launches = 0; h->last_cuda = 0; h->smem_configured = false;
-  h->prof_mask = 0; h->prof_used = 0;
+  h->prof_mask = 0; h->prof_used = 0; h->encode_tiled = nullptr;
 
   // block sizes: defaults, then shrink until the plan fits the cap
   h->bL = std::min<int64_t>(NL, (opt && opt->bL) ? opt->bL : 32);
@@ -453,11 +454,12 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
 
 int thc_destroy(thc_handle* h) {
   if (!h) return THC_ERR_INVALID_ARG;
-  if ((h->ws && h->ws_owned) || !h->prof_events.empty()) {
+  if ((h->ws && h->ws_owned) || !h->prof_events.empty() || !h->tp_lists.empty()) {
     DeviceGuard g(h->device);
     cudaStreamSynchronize(h->stream);
     if (h->ws && h->ws_owned) cudaFree(h->ws);
     for (cudaEvent_t e : h->prof_events) cudaEventDestroy(e);
+    for (auto& l : h->tp_lists) cudaFree(l.dev);
   }
   delete h;
   return THC_OK;
@@ -549,10 +551,14 @@ int thc_profile_end(thc_handle* h, double ms[3], int64_t counts[3]) {
   for (int k = 0; k < 3; k++) { ms[k] = 0.0; counts[k] = 0; }
   cudaError_t e = cudaStreamSynchronize(h->stream);
   if (e != cudaSuccess) { h->last_cuda = (int)e; return THC_ERR_CUDA; }
+  const bool trace = getenv("THC_TRACE") != nullptr;     // developer aid: one stderr line per timed launch
   for (size_t k = 0; k < h->prof_used; k++) {
     float t = 0.f;
     e = cudaEventElapsedTime(&t, h->prof_events[2 * k], h->prof_events[2 * k + 1]);
     if (e != cudaSuccess) { h->last_cuda = (int)e; return THC_ERR_CUDA; }
+    if (trace)
+      fprintf(stderr, "[thc trace] %9.4f ms  %8.3f T(fl)op/s-or-Gelem/s  %s\n", t, h->prof_flops[k] / (t * 1e-3) / 1e12,
+              h->prof_desc[k].c_str());
     ms[h->prof_class[k]] += (double)t;
     counts[h->prof_class[k]]++;
   }

@@ -1,0 +1,261 @@
+// Alg.6 line 11, the rate-limiting step of the THC ladder-type T2^2 terms ("implemented with a custom
+// CUDA kernel", l.257):
+//
+//     H[p][q][r] (+)= sum_I ( E_I[p][q] F_I[p][r] + E_I[p][r] F_I[p][q] ) G_I[q][r]
+//
+// This is a three-way "triangle" product (every factor carries two of the three output indices and the summed index),
+// not a dense contraction: it runs on the FP64 FMA pipe.  Work per (p,q,r,I):
+//   the bracket s_I[p](q,r) is symmetric in (q,r), so a CTA that owns the block (p-tile, q-tile, r-tile) with the q-tile
+//   outside the r-tile also owns the mirrored block (p-tile, r-tile, q-tile): s is formed once (DMUL + DFMA) and used
+//   twice (2 DFMA) -> 2 FP64 instructions per (p,q,r,I) instead of 3.  CTAs whose q-tile lies inside their r-tile
+//   ("diagonal") do the plain 3-instruction update of the direct block only.
+//
+// B200 design
+//   * persistent CTAs (one per SM, 256 threads = 8 warps as 2p x 2q x 2r; lane = 2p x 4q x 4r; thread tile 4p x 2q x 4r
+//     plus its mirror = 64 FP64 accumulators), CTA tile 16p x 16q x 32r (+ mirror 16p x 32r x 16q);
+//   * operands are fetched by TMA (cp.async.bulk.tensor.3d, SWIZZLE_128B) as ten 16x16 FP64 blocks (2 KB each) per grid
+//     point I into a TP_STAGES-deep shared-memory ring; full/empty mbarriers, no __syncthreads in the I loop.  The TMA
+//     issue is done by lane 0 of warp (j mod 8) at iteration j, for iteration j + TP_STAGES - 2 (two iterations of slack
+//     on the empty barrier), so the ring keeps ~120 KB in flight per SM;
+//   * the 128-byte swizzle makes every 16-byte fragment load bank-conflict free (rows 4 apart differ in chunk bit 2);
+//   * work items (p-tile, q-tile, r-tile) come from a host-built list ordered in groups of 8 p-tiles x 6 q-tiles x 3
+//     r-tiles, so that the ~148 CTAs running at the same time share their operand tiles in L2 (5x less HBM traffic).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace thc {
+
+constexpr int TP_PT = 16, TP_QT = 16, TP_RT = 32;
+constexpr int TP_STAGES = 8, TP_LOOKAHEAD = TP_STAGES - 2;
+constexpr int TP_BLK_BYTES = 16 * 16 * 8;                  // one 16x16 FP64 block
+constexpr int TP_STAGE_BYTES = 10 * TP_BLK_BYTES;          // EPQ FPQ EPR0 EPR1 FPR0 FPR1 GQR0 GQR1 GRQ0 GRQ1
+constexpr int TP_SMEM_BYTES = TP_STAGES * TP_STAGE_BYTES + 1024 /* alignment slack */ + 2 * TP_STAGES * 8;
+constexpr int TP_THREADS = 256;
+
+struct TripleItem { int p0, q0, r0, diag; };
+
+struct TripleParams {
+  double* H;
+  const TripleItem* items;
+  int n_items;
+  int nI, nPp, NPp;        // padded extents: nPp % 16 == 0, NPp % 32 == 0
+  int accumulate;
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, int bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+      : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  while (!mbar_try_wait(bar, parity)) {}
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+      ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
+}
+__device__ __forceinline__ double2 lds128(const uint8_t* base, uint32_t off) {
+  return *reinterpret_cast<const double2*>(base + off);
+}
+
+// E, F: tensor maps over [nI][nPp][NPp] (innermost NPp), G: over [nI][NPp][NPp]; box 16 x 16 x 1, SWIZZLE_128B.
+__global__ void __launch_bounds__(TP_THREADS, 1)
+triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_constant__ CUtensorMap mapF,
+                      const __grid_constant__ CUtensorMap mapG, const TripleParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t ring = (smem_u32(smem_raw) + 1023u) & ~1023u;          // 1024-byte aligned (swizzle atom)
+  const uint8_t* ring_ptr = smem_raw + (ring - smem_u32(smem_raw));
+  const uint32_t bar_full = ring + TP_STAGES * TP_STAGE_BYTES;
+  const uint32_t bar_empty = bar_full + TP_STAGES * 8;
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int wp = warp >> 2, wq = (warp >> 1) & 1, wr = warp & 1;
+  const int lp = lane >> 4, lq = (lane >> 2) & 3, lr = lane & 3;
+  const int tp0 = wp * 8 + lp * 4;                      // 4 consecutive p
+  const int tq0 = wq * 8 + lq * 2;                      // 2 consecutive q
+  const int cq = tq0 >> 1;                              // 16-byte chunk of (.., tq0) in a 16-wide row
+  // r: this thread owns r = wr*16 + {2 lr, 2 lr + 1, 2 lr + 8, 2 lr + 9}  -> block wr, chunks lr and lr + 4
+
+  const int my_items = p.n_items > (int)blockIdx.x ? (p.n_items - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
+  const int total = my_items * p.nI;          // < 2^31 (checked by the launcher)
+
+  if (tid == 0) {
+    for (int s = 0; s < TP_STAGES; s++) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, 8); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+
+  // ---- producer side (lane 0 of each warp takes every 8th iteration) -------------------------------------------------
+  auto issue = [&](int jn, int k, int I) {          // fill for flat iteration jn = (item k of this CTA, grid point I)
+    const TripleItem it = p.items[blockIdx.x + (long long)k * gridDim.x];
+    const int s = jn % TP_STAGES;
+    const uint32_t dst = ring + s * TP_STAGE_BYTES, bf = bar_full + 8 * s;
+    mbar_expect_tx(bf, it.diag ? 8 * TP_BLK_BYTES : 10 * TP_BLK_BYTES);
+    tma_load_3d(dst + 0 * TP_BLK_BYTES, &mapE, it.q0, it.p0, I, bf);
+    tma_load_3d(dst + 1 * TP_BLK_BYTES, &mapF, it.q0, it.p0, I, bf);
+    tma_load_3d(dst + 2 * TP_BLK_BYTES, &mapE, it.r0, it.p0, I, bf);
+    tma_load_3d(dst + 3 * TP_BLK_BYTES, &mapE, it.r0 + 16, it.p0, I, bf);
+    tma_load_3d(dst + 4 * TP_BLK_BYTES, &mapF, it.r0, it.p0, I, bf);
+    tma_load_3d(dst + 5 * TP_BLK_BYTES, &mapF, it.r0 + 16, it.p0, I, bf);
+    tma_load_3d(dst + 6 * TP_BLK_BYTES, &mapG, it.r0, it.q0, I, bf);
+    tma_load_3d(dst + 7 * TP_BLK_BYTES, &mapG, it.r0 + 16, it.q0, I, bf);
+    if (!it.diag) {
+      tma_load_3d(dst + 8 * TP_BLK_BYTES, &mapG, it.q0, it.r0, I, bf);
+      tma_load_3d(dst + 9 * TP_BLK_BYTES, &mapG, it.q0, it.r0 + 16, I, bf);
+    }
+  };
+  if (tid == 0) {
+    int k = 0, I = 0;
+    for (int jn = 0; jn < TP_LOOKAHEAD && jn < total; jn++) {
+      issue(jn, k, I);
+      if (++I == p.nI) { I = 0; k++; }
+    }
+  }
+  // this warp refills iterations jn = warp + TP_LOOKAHEAD + 8 m
+  int pj = warp + TP_LOOKAHEAD;
+  int pk = pj / p.nI, pI = pj % p.nI;
+
+  // ---- per-thread shared-memory byte offsets inside a stage (swizzle: chunk ^= row & 7) ------------------------------
+  uint32_t offPQ[4], offPR[4], offQR[2], offRQ[2];
+#pragma unroll
+  for (int a = 0; a < 4; a++) {
+    const int row = tp0 + a;
+    offPQ[a] = row * 128 + ((cq ^ (row & 7)) << 4);
+    offPR[a] = (2 + wr) * TP_BLK_BYTES + row * 128 + ((lr ^ (row & 7)) << 4);        // chunk lr; chunk lr + 4 is ^ 64
+  }
+#pragma unroll
+  for (int b = 0; b < 2; b++) {
+    const int row = tq0 + b;
+    offQR[b] = (6 + wr) * TP_BLK_BYTES + row * 128 + ((lr ^ (row & 7)) << 4);
+    const int rr = 2 * lr + b;                                                         // rows rr and rr + 8 of block 8 + wr
+    offRQ[b] = (8 + wr) * TP_BLK_BYTES + rr * 128 + ((cq ^ (rr & 7)) << 4);
+  }
+
+  double hqr[4][2][4], hrq[4][2][4];
+  int I = 0, k = 0;
+  TripleItem cur = my_items > 0 ? p.items[blockIdx.x] : TripleItem{0, 0, 0, 1};
+
+  for (int j = 0; j < total; j++) {
+    if (I == 0) {
+#pragma unroll
+      for (int a = 0; a < 4; a++)
+#pragma unroll
+        for (int b = 0; b < 2; b++)
+#pragma unroll
+          for (int c = 0; c < 4; c++) hqr[a][b][c] = hrq[a][b][c] = 0.0;
+    }
+    const int s = j % TP_STAGES;
+    const uint32_t par = (uint32_t)((j / TP_STAGES) & 1);
+    mbar_wait(bar_full + 8 * s, par);
+
+    // refill (two iterations behind the consumers)
+    if ((j & 7) == warp) {
+      if (lane == 0 && pj < total) {
+        const int sn = pj % TP_STAGES;
+        const int fill = pj / TP_STAGES;
+        if (fill > 0) mbar_wait(bar_empty + 8 * sn, (uint32_t)((fill - 1) & 1));
+        issue(pj, pk, pI);
+      }
+      pj += 8; pI += 8;
+      while (pI >= p.nI) { pI -= p.nI; pk++; }
+      __syncwarp();
+    }
+
+    const uint8_t* st = ring_ptr + s * TP_STAGE_BYTES;
+    double gqr[2][4], grq[4][2];
+#pragma unroll
+    for (int b = 0; b < 2; b++) {
+      double2 g0 = lds128(st, offQR[b]), g1 = lds128(st, (offQR[b] ^ 64));
+      gqr[b][0] = g0.x; gqr[b][1] = g0.y; gqr[b][2] = g1.x; gqr[b][3] = g1.y;
+    }
+    if (!cur.diag) {
+#pragma unroll
+      for (int c = 0; c < 4; c++) {
+        double2 gg = lds128(st, offRQ[c & 1] + (c >> 1) * 1024);
+        grq[c][0] = gg.x; grq[c][1] = gg.y;
+      }
+#pragma unroll
+      for (int a = 0; a < 4; a++) {
+        double2 e = lds128(st, offPQ[a]), f = lds128(st, TP_BLK_BYTES + offPQ[a]);
+        double2 e0 = lds128(st, offPR[a]), e1 = lds128(st, (offPR[a] ^ 64));
+        double2 f0 = lds128(st, 2 * TP_BLK_BYTES + offPR[a]), f1 = lds128(st, 2 * TP_BLK_BYTES + (offPR[a] ^ 64));
+        const double epq[2] = {e.x, e.y}, fpq[2] = {f.x, f.y};
+        const double epr[4] = {e0.x, e0.y, e1.x, e1.y}, fpr[4] = {f0.x, f0.y, f1.x, f1.y};
+#pragma unroll
+        for (int b = 0; b < 2; b++)
+#pragma unroll
+          for (int c = 0; c < 4; c++) {
+            const double sv = fma(epr[c], fpq[b], epq[b] * fpr[c]);
+            hqr[a][b][c] = fma(sv, gqr[b][c], hqr[a][b][c]);
+            hrq[a][b][c] = fma(sv, grq[c][b], hrq[a][b][c]);
+          }
+      }
+    } else {
+#pragma unroll
+      for (int a = 0; a < 4; a++) {
+        double2 e = lds128(st, offPQ[a]), f = lds128(st, TP_BLK_BYTES + offPQ[a]);
+        double2 e0 = lds128(st, offPR[a]), e1 = lds128(st, (offPR[a] ^ 64));
+        double2 f0 = lds128(st, 2 * TP_BLK_BYTES + offPR[a]), f1 = lds128(st, 2 * TP_BLK_BYTES + (offPR[a] ^ 64));
+        const double epq[2] = {e.x, e.y}, fpq[2] = {f.x, f.y};
+        const double epr[4] = {e0.x, e0.y, e1.x, e1.y}, fpr[4] = {f0.x, f0.y, f1.x, f1.y};
+#pragma unroll
+        for (int b = 0; b < 2; b++)
+#pragma unroll
+          for (int c = 0; c < 4; c++) {
+            const double sv = fma(epr[c], fpq[b], epq[b] * fpr[c]);
+            hqr[a][b][c] = fma(sv, gqr[b][c], hqr[a][b][c]);
+          }
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar_empty + 8 * s);
+
+    if (++I == p.nI) {
+      // ---- write back this item's block(s) of H[p][q][r] -----------------------------------------------------------
+      const long long sHp = (long long)p.NPp * p.NPp;
+      const int rA = cur.r0 + wr * 16 + 2 * lr;              // r = rA, rA + 1, rA + 8, rA + 9
+#pragma unroll
+      for (int a = 0; a < 4; a++) {
+        double* Hp = p.H + (long long)(cur.p0 + tp0 + a) * sHp;
+#pragma unroll
+        for (int b = 0; b < 2; b++) {
+          double* row = Hp + (long long)(cur.q0 + tq0 + b) * p.NPp;
+          double2* d0 = reinterpret_cast<double2*>(row + rA);
+          double2* d1 = reinterpret_cast<double2*>(row + rA + 8);
+          double2 v0 = make_double2(hqr[a][b][0], hqr[a][b][1]), v1 = make_double2(hqr[a][b][2], hqr[a][b][3]);
+          if (p.accumulate) { double2 o0 = *d0, o1 = *d1; v0.x += o0.x; v0.y += o0.y; v1.x += o1.x; v1.y += o1.y; }
+          *d0 = v0; *d1 = v1;
+        }
+        if (!cur.diag) {
+#pragma unroll
+          for (int c = 0; c < 4; c++) {
+            const int r = rA + (c & 1) + 8 * (c >> 1);
+            double2* d = reinterpret_cast<double2*>(Hp + (long long)r * p.NPp + cur.q0 + tq0);
+            double2 vv = make_double2(hrq[a][0][c], hrq[a][1][c]);
+            if (p.accumulate) { double2 o = *d; vv.x += o.x; vv.y += o.y; }
+            *d = vv;
+          }
+        }
+      }
+      I = 0; k++;
+      if (k < my_items) cur = p.items[blockIdx.x + (long long)k * gridDim.x];
+    }
+  }
+}
+
+}  // namespace thc
