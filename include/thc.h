@@ -136,10 +136,11 @@ int thc_dgemm(thc_handle* h, int a_kmajor, int b_kmajor, int64_t M, int64_t N, i
 
 /* Alg.6 line 11 (l.714) alone, for tests and roofline measurement:
  * H[p][q][r] (+)= sum_I (E[I][p][q] F[I][p][r] + E[I][p][r] F[I][p][q]) G[I][q][r]
- * E, F: [nI][nPp][NPp], G: [nI][NPp][NPp], H: [nPp][NPp][NPp]; NPp a multiple of 32, nPp of 16 (padded
- * extents; padded entries are computed from whatever the padding holds and must be ignored).           */
+ * E, F: [nI][nPp][NPp], G, GT: [nI][NPp][NPp] with GT[I][q][r] = G[I][r][q] (the caller supplies both orientations;
+ * the kernel reads the mirrored block from GT), H: [nPp][NPp][NPp]; NPp a multiple of 32, nPp of 16 (padded extents;
+ * padded entries are computed from whatever the padding holds and must be ignored).  All pointers 16-byte aligned. */
 int thc_triple_product(thc_handle* h, int64_t nI, int64_t nPp, int64_t NPp, const double* E, const double* F,
-                       const double* G, double* H, int accumulate);
+                       const double* G, const double* GT, double* H, int accumulate);
 
 const char* thc_strerror(int status);
 int thc_last_cuda_error(const thc_handle* h);   /* the cudaError_t of the last THC_ERR_CUDA, else 0 */

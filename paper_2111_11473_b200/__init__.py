@@ -88,7 +88,7 @@ def lib() -> ctypes.CDLL:
     L.thc_algorithmic_flops.argtypes = [VP]
     L.thc_algorithmic_flops.restype = D
     L.thc_dgemm.argtypes = [VP, ctypes.c_int, ctypes.c_int, I64, I64, I64, D, P, I64, P, I64, D, P, I64]
-    L.thc_triple_product.argtypes = [VP, I64, I64, I64, P, P, P, P, ctypes.c_int]
+    L.thc_triple_product.argtypes = [VP, I64, I64, I64, P, P, P, P, P, ctypes.c_int]
     L.thc_strerror.argtypes = [ctypes.c_int]
     L.thc_strerror.restype = ctypes.c_char_p
     L.thc_last_cuda_error.argtypes = [VP]
@@ -141,8 +141,8 @@ class Thc:
         self._device = torch.device("cuda", torch.cuda.current_device() if device < 0 else device)
 
     def close(self):
-        if getattr(self, "_h", None) is not None and self._h.value:
-            lib().thc_destroy(self._h)
+        if getattr(self, "_h", None) is not None and self._h.value and _lib is not None:
+            _lib.thc_destroy(self._h)
             self._h = ctypes.c_void_p()
             self._ws = None
 
@@ -253,10 +253,10 @@ class Thc:
         _check(lib().thc_dgemm(self._h, int(a_kmajor), int(b_kmajor), M, N, K, alpha, _dev_ptr(A, "A"), lda,
                                _dev_ptr(B, "B"), ldb, beta, _dev_ptr(C, "C"), ldc), self._h)
 
-    def thc_triple_product(self, nI, nPp, NPp, E, F, G, H, accumulate):
+    def thc_triple_product(self, nI, nPp, NPp, E, F, G, GT, H, accumulate):
         self._prepare(self.workspace_bytes)
         _check(lib().thc_triple_product(self._h, nI, nPp, NPp, _dev_ptr(E, "E", nI * nPp * NPp),
-                                        _dev_ptr(F, "F", nI * nPp * NPp), _dev_ptr(G, "G", nI * NPp * NPp),
+                                        _dev_ptr(F, "F", nI * nPp * NPp), _dev_ptr(G, "G", nI * NPp * NPp), _dev_ptr(GT, "GT", nI * NPp * NPp),
                                         _dev_ptr(H, "H", nPp * NPp * NPp), int(accumulate)), self._h)
 
 

@@ -335,22 +335,23 @@ struct Ctx {
     h->tp_lists.push_back(l);
     return &h->tp_lists.back();
   }
-  void triple_product(const double* E, const double* F, const double* G, double* H, i64 nI, i64 nPp, i64 NPp, int accumulate) {
+  void triple_product(const double* E, const double* F, const double* G, const double* GT, double* H, i64 nI, i64 nPp, i64 NPp, int accumulate) {
     if (dry || !ok()) return;
     if (!h->smem_configured) {
       check(cudaFuncSetAttribute(triple_product_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TP_SMEM_BYTES));
       h->smem_configured = true;
     }
     const thc_handle::TripleList* list = triple_items(nPp, NPp);
-    CUtensorMap mE, mF, mG;
-    if (!list || !make_map3(&mE, E, NPp, nPp, nI) || !make_map3(&mF, F, NPp, nPp, nI) || !make_map3(&mG, G, NPp, NPp, nI)) return;
+    CUtensorMap mE, mF, mG, mGT;
+    if (!list || !make_map3(&mE, E, NPp, nPp, nI) || !make_map3(&mF, F, NPp, nPp, nI) || !make_map3(&mG, G, NPp, NPp, nI) ||
+        !make_map3(&mGT, GT, NPp, NPp, nI)) return;
     TripleParams p;
     p.H = H; p.items = list->dev; p.n_items = list->n;
     p.nI = (int)nI; p.nPp = (int)nPp; p.NPp = (int)NPp; p.accumulate = accumulate;
     const int grid = std::min(list->n, h->sms);
     if (((i64)(list->n + grid - 1) / grid) * nI >= ((i64)1 << 31)) { status = THC_ERR_OVERFLOW; return; }
     prof_start(1, "triple_product", 5.0 * nI * nPp * (double)NPp * NPp);
-    triple_product_kernel<<<grid, TP_THREADS, TP_SMEM_BYTES, h->stream>>>(mE, mF, mG, p);
+    triple_product_kernel<<<grid, TP_THREADS, TP_SMEM_BYTES, h->stream>>>(mE, mF, mG, mGT, p);
     launched();
     prof_stop(1);
   }

@@ -233,18 +233,20 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out) {
       for (i64 I0 = 0; I0 < NX; I0 += h->bI) {
         const i64 ni = std::min<i64>(h->bI, NX - I0), m2 = ar.mark();
         // line 2/7: BI[I][i][a] = sum_J V[I,J] Yo[i,J] Yv[a,J]
-        double *VY = ar.alloc(ni * o * NX), *BI = ar.alloc(ni * ov), *GXT = ar.alloc(ni * NP * o), *Gt = ar.alloc(ni * NPp * NPp);
+        double *VY = ar.alloc(ni * o * NX), *BI = ar.alloc(ni * ov), *GXT = ar.alloc(ni * NP * o), *Gt = ar.alloc(ni * NPp * NPp), *GtT = ar.alloc(ni * NPp * NPp);
         double *Eb = ar.alloc(ni * bXp * NPp), *Fb = ar.alloc(ni * bXp * NPp);
         c.rowscale(Yo, NX, in.V + I0 * NX, NX, nullptr, 1.0, VY, ni, o, NX);
         c.gemm(Gemm(VY, NX, 'K', Yv, NX, 'K', BI, v, ni * o, v, NX));
         // line 10: G_I[q][r] = sum_ia Xo[i,q] Xv[a,r] BI[I][i][a]
         c.gemm(Gemm(XvT, v, 'K', BI, v, 'K', GXT, o, NP, o, v).batch(ni, 0, ov, NP * o));
         c.gemm(Gemm(XoT, o, 'K', GXT, o, 'K', Gt, NPp, NP, NP, o).batch(ni, 0, NP * o, NPp * NPp));
+        // and its transpose GtT_I[q][r] = G_I[r][q] (operands swapped), read by the mirrored half of line 11
+        c.gemm(Gemm(GXT, o, 'K', XoT, o, 'K', GtT, NPp, NP, NP, o).batch(ni, NP * o, 0, NPp * NPp));
         // lines 8-9: E_I[p][q] = sum_i Cc[p][(q,i)] Yo[i,I] ;  F_I[p][r] = sum_a Dd[p][(r,a)] Yv[a,I]
         c.gemm(Gemm(YoT + I0 * o, o, 'K', Cc, o, 'K', Eb, bXp * NPp, ni, NP, o).batch(npb, 0, NP * o, NPp));
         c.gemm(Gemm(YvT + I0 * v, v, 'K', Dd, v, 'K', Fb, bXp * NPp, ni, NP, v).batch(npb, 0, NP * v, NPp));
         // line 11
-        c.triple_product(Eb, Fb, Gt, H, ni, bXp, NPp, first ? 0 : 1);
+        c.triple_product(Eb, Fb, Gt, GtT, H, ni, bXp, NPp, first ? 0 : 1);
         first = false;
         ar.release(m2);
       }
@@ -428,7 +430,7 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
   const int64_t p7_auto = std::max<int64_t>(1, ((int64_t)2 << 30) / (NX * NX * 8));
   h->bP7 = std::min<int64_t>(NP, (opt && opt->bP7) ? opt->bP7 : p7_auto);
   h->bX = std::min<int64_t>(pad_to(NP, 16), (opt && opt->bX) ? pad_to(opt->bX, 16) : pad_to(NP, 16));
-  h->bI = std::min<int64_t>(NX, (opt && opt->bI) ? opt->bI : 64);
+  h->bI = std::min<int64_t>(NX, (opt && opt->bI) ? opt->bI : 512);   // long I loops amortise the H read-modify-write
   int64_t cap = opt ? opt->workspace_bytes_max : 0;
   if (cap == 0) {
     DeviceGuard g(dev);
@@ -440,7 +442,9 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
   for (;;) {
     h->need_bytes = need_device(h);
     if (h->need_bytes <= cap) break;
-    if (!fix_bX && h->bX > 64) h->bX = pad_to(h->bX / 2, 16);
+    if (!fix_bX && h->bX > 512) h->bX = pad_to(h->bX / 2, 16);
+    else if (!fix_bI && h->bI > 128) h->bI = h->bI / 2;
+    else if (!fix_bX && h->bX > 64) h->bX = pad_to(h->bX / 2, 16);
     else if (!fix_bP7 && h->bP7 > 1) h->bP7 = h->bP7 / 2;
     else if (!fix_bL && h->bL > 4) h->bL = h->bL / 2;
     else if (!fix_bI && h->bI > 16) h->bI = h->bI / 2;
@@ -660,17 +664,17 @@ int thc_dgemm(thc_handle* h, int a_kmajor, int b_kmajor, int64_t M, int64_t N, i
 }
 
 int thc_triple_product(thc_handle* h, int64_t nI, int64_t nPp, int64_t NPp, const double* E, const double* F,
-                       const double* G, double* H, int accumulate) {
-  if (!h || bad_ptr(E) || bad_ptr(F) || bad_ptr(G) || bad_ptr(H) || nI <= 0 || nPp <= 0 || NPp <= 0) return THC_ERR_INVALID_ARG;
+                       const double* G, const double* GT, double* H, int accumulate) {
+  if (!h || bad_ptr(E) || bad_ptr(F) || bad_ptr(G) || bad_ptr(GT) || bad_ptr(H) || nI <= 0 || nPp <= 0 || NPp <= 0) return THC_ERR_INVALID_ARG;
   if (nPp % thc::TP_PT != 0 || NPp % thc::TP_RT != 0) return THC_ERR_INVALID_ARG;
-  if (((reinterpret_cast<uintptr_t>(E) | reinterpret_cast<uintptr_t>(F) | reinterpret_cast<uintptr_t>(G) |
+  if (((reinterpret_cast<uintptr_t>(E) | reinterpret_cast<uintptr_t>(F) | reinterpret_cast<uintptr_t>(G) | reinterpret_cast<uintptr_t>(GT) |
         reinterpret_cast<uintptr_t>(H)) & 15) != 0)
     return THC_ERR_INVALID_ARG;
   DeviceGuard g(h->device);
   if (!g.ok) return THC_ERR_CUDA;
   Ctx c{h};
   c.dry = false;
-  c.triple_product(E, F, G, H, nI, nPp, NPp, accumulate);
+  c.triple_product(E, F, G, GT, H, nI, nPp, NPp, accumulate);
   return c.status;
 }
 

@@ -30,7 +30,7 @@ namespace thc {
 constexpr int TP_PT = 16, TP_QT = 16, TP_RT = 32;
 constexpr int TP_STAGES = 8, TP_LOOKAHEAD = TP_STAGES - 2;
 constexpr int TP_BLK_BYTES = 16 * 16 * 8;                  // one 16x16 FP64 block
-constexpr int TP_STAGE_BYTES = 10 * TP_BLK_BYTES;          // EPQ FPQ EPR0 EPR1 FPR0 FPR1 GQR0 GQR1 GRQ0 GRQ1
+constexpr int TP_STAGE_BYTES = 10 * TP_BLK_BYTES;          // EPQ FPQ EPR0 EPR1 FPR0 FPR1 GQR0 GQR1 GTQR0 GTQR1
 constexpr int TP_SMEM_BYTES = TP_STAGES * TP_STAGE_BYTES + 1024 /* alignment slack */ + 2 * TP_STAGES * 8;
 constexpr int TP_THREADS = 256;
 
@@ -73,10 +73,12 @@ __device__ __forceinline__ double2 lds128(const uint8_t* base, uint32_t off) {
   return *reinterpret_cast<const double2*>(base + off);
 }
 
-// E, F: tensor maps over [nI][nPp][NPp] (innermost NPp), G: over [nI][NPp][NPp]; box 16 x 16 x 1, SWIZZLE_128B.
+// E, F: tensor maps over [nI][nPp][NPp] (innermost NPp); G, GT: over [nI][NPp][NPp] with GT_I[q][r] = G_I[r][q] (so that the
+// mirrored block is read with the same row-q / chunk-r pattern as the direct one); box 16 x 16 x 1, SWIZZLE_128B.
 __global__ void __launch_bounds__(TP_THREADS, 1)
 triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_constant__ CUtensorMap mapF,
-                      const __grid_constant__ CUtensorMap mapG, const TripleParams p) {
+                      const __grid_constant__ CUtensorMap mapG, const __grid_constant__ CUtensorMap mapGT,
+                      const TripleParams p) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t ring = (smem_u32(smem_raw) + 1023u) & ~1023u;          // 1024-byte aligned (swizzle atom)
   const uint8_t* ring_ptr = smem_raw + (ring - smem_u32(smem_raw));
@@ -85,7 +87,7 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int wp = warp >> 2, wq = (warp >> 1) & 1, wr = warp & 1;
-  const int lp = lane >> 4, lq = (lane >> 2) & 3, lr = lane & 3;
+  const int lp = lane >> 4, lq = ((lane >> 2) & 1) * 2 + ((lane >> 3) & 1), lr = lane & 3;   // lane bit 2 -> q bit 2
   const int tp0 = wp * 8 + lp * 4;                      // 4 consecutive p
   const int tq0 = wq * 8 + lq * 2;                      // 2 consecutive q
   const int cq = tq0 >> 1;                              // 16-byte chunk of (.., tq0) in a 16-wide row
@@ -115,8 +117,8 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
     tma_load_3d(dst + 6 * TP_BLK_BYTES, &mapG, it.r0, it.q0, I, bf);
     tma_load_3d(dst + 7 * TP_BLK_BYTES, &mapG, it.r0 + 16, it.q0, I, bf);
     if (!it.diag) {
-      tma_load_3d(dst + 8 * TP_BLK_BYTES, &mapG, it.q0, it.r0, I, bf);
-      tma_load_3d(dst + 9 * TP_BLK_BYTES, &mapG, it.q0, it.r0 + 16, I, bf);
+      tma_load_3d(dst + 8 * TP_BLK_BYTES, &mapGT, it.r0, it.q0, I, bf);
+      tma_load_3d(dst + 9 * TP_BLK_BYTES, &mapGT, it.r0 + 16, it.q0, I, bf);
     }
   };
   if (tid == 0) {
@@ -131,7 +133,7 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
   int pk = pj / p.nI, pI = pj % p.nI;
 
   // ---- per-thread shared-memory byte offsets inside a stage (swizzle: chunk ^= row & 7) ------------------------------
-  uint32_t offPQ[4], offPR[4], offQR[2], offRQ[2];
+  uint32_t offPQ[4], offPR[4], offQR[2];
 #pragma unroll
   for (int a = 0; a < 4; a++) {
     const int row = tp0 + a;
@@ -142,11 +144,9 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
   for (int b = 0; b < 2; b++) {
     const int row = tq0 + b;
     offQR[b] = (6 + wr) * TP_BLK_BYTES + row * 128 + ((lr ^ (row & 7)) << 4);
-    const int rr = 2 * lr + b;                                                         // rows rr and rr + 8 of block 8 + wr
-    offRQ[b] = (8 + wr) * TP_BLK_BYTES + rr * 128 + ((cq ^ (rr & 7)) << 4);
   }
 
-  double hqr[4][2][4], hrq[4][2][4];
+  double hqr[4][2][4], hrq[4][2][4];      // hrq[a][b][c] accumulates H[p_a][r_c][q_b]
   int I = 0, k = 0;
   TripleItem cur = my_items > 0 ? p.items[blockIdx.x] : TripleItem{0, 0, 0, 1};
 
@@ -177,7 +177,7 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
     }
 
     const uint8_t* st = ring_ptr + s * TP_STAGE_BYTES;
-    double gqr[2][4], grq[4][2];
+    double gqr[2][4], gt[2][4];            // gt[b][c] = G_I[r_c][q_b] (read from the transposed copy GT_I[q][r])
 #pragma unroll
     for (int b = 0; b < 2; b++) {
       double2 g0 = lds128(st, offQR[b]), g1 = lds128(st, (offQR[b] ^ 64));
@@ -185,9 +185,9 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
     }
     if (!cur.diag) {
 #pragma unroll
-      for (int c = 0; c < 4; c++) {
-        double2 gg = lds128(st, offRQ[c & 1] + (c >> 1) * 1024);
-        grq[c][0] = gg.x; grq[c][1] = gg.y;
+      for (int b = 0; b < 2; b++) {
+        double2 g0 = lds128(st, 2 * TP_BLK_BYTES + offQR[b]), g1 = lds128(st, 2 * TP_BLK_BYTES + (offQR[b] ^ 64));
+        gt[b][0] = g0.x; gt[b][1] = g0.y; gt[b][2] = g1.x; gt[b][3] = g1.y;
       }
 #pragma unroll
       for (int a = 0; a < 4; a++) {
@@ -202,7 +202,7 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
           for (int c = 0; c < 4; c++) {
             const double sv = fma(epr[c], fpq[b], epq[b] * fpr[c]);
             hqr[a][b][c] = fma(sv, gqr[b][c], hqr[a][b][c]);
-            hrq[a][b][c] = fma(sv, grq[c][b], hrq[a][b][c]);
+            hrq[a][b][c] = fma(sv, gt[b][c], hrq[a][b][c]);
           }
       }
     } else {
