@@ -44,39 +44,57 @@ __device__ __forceinline__ void cp_async8(void* smem, const void* gmem, int src_
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N)); }
 
-// Copy one BK-deep slab of an operand tile (ROWS rows starting at row0 of an operand with `nrows` rows) into smem.
+// Per-thread state for copying one BK-deep slab of an operand tile (ROWS rows of an operand with `nrows` rows) into shared
+// memory.  Every index computation (chunk -> row / k offset, row bounds, smem offset) is done once in init(); issuing a
+// slab costs a pointer add and a K-tail clamp per 16-byte chunk, so the warps spend their issue slots on DMMA.
+//   K-major operand: smem [BK/8][ROWS][8], global element (r, k) at g[r*ld + k]
+//   M/N-major      : smem [BK][ROWS+2],    global element (r, k) at g[k*ld + r]
 template <int ROWS, int BK, int NTHREADS, bool KMAJOR, bool AL16>
-__device__ __forceinline__ void load_tile(double* s, const double* __restrict__ g, long long ld, int row0, int nrows,
-                                          int k0, int K, int tid) {
-  if (KMAJOR) {
-    // smem [BK/8][ROWS][8]; global row r: g[r*ld + k]
-    constexpr int CHUNKS = ROWS * BK / 2;
-    for (int c = tid; c < CHUNKS; c += NTHREADS) {
-      int kb8 = c / (ROWS * 4), rem = c % (ROWS * 4), r = rem / 4, cc = rem % 4;
-      int k = k0 + kb8 * 8 + cc * 2;
-      int row = row0 + r;
-      double* dst = s + (kb8 * ROWS + r) * 8 + cc * 2;
-      bool rok = row < nrows;
-      const double* src = g + (rok ? (long long)row * ld : 0) + (k < K ? k : 0);
-      int nb = rok ? max(0, min(2, K - k)) * 8 : 0;
-      if (AL16) {
-        cp_async16(dst, src, nb);
+struct TileLoader {
+  static constexpr int CHUNKS = ROWS * BK / 2;
+  static constexpr int NCH = (CHUNKS + NTHREADS - 1) / NTHREADS;
+  long long goff[NCH];   // global offset of the chunk in k-tile 0 (doubles)
+  int soff[NCH];         // shared offset inside a stage (doubles)
+  int kofs[NCH];         // k offset inside the tile
+  int bytes[NCH];        // bytes the chunk may copy as far as the row bound is concerned (0, 8 or 16)
+  long long kstep;       // global offset between consecutive k-tiles
+  __device__ __forceinline__ void init(long long ld, int row0, int nrows, int tid) {
+#pragma unroll
+    for (int q = 0; q < NCH; q++) {
+      const int c = tid + q * NTHREADS;
+      if (KMAJOR) {
+        const int kb8 = c / (ROWS * 4), rem = c % (ROWS * 4), r = rem / 4, cc = rem % 4;
+        const int row = row0 + r;
+        const bool ok = c < CHUNKS && row < nrows;
+        soff[q] = (kb8 * ROWS + r) * 8 + cc * 2;
+        kofs[q] = kb8 * 8 + cc * 2;
+        goff[q] = (ok ? (long long)row * ld : 0) + kofs[q];
+        bytes[q] = ok ? 16 : 0;
       } else {
-        cp_async8(dst, src, nb >= 8 ? 8 : 0);
-        cp_async8(dst + 1, nb >= 16 ? src + 1 : src, nb >= 16 ? 8 : 0);
+        const int kk = c / (ROWS / 2), cc = c % (ROWS / 2);
+        const int row = row0 + cc * 2;
+        const bool ok = c < CHUNKS;
+        soff[q] = kk * (ROWS + 2) + cc * 2;
+        kofs[q] = kk;
+        goff[q] = (long long)kk * ld + (row < nrows ? row : 0);
+        bytes[q] = ok ? max(0, min(2, nrows - row)) * 8 : 0;
       }
     }
-  } else {
-    // smem [BK][ROWS+2]; global: g[k*ld + r]
-    constexpr int PITCH = ROWS + 2;
-    constexpr int CHUNKS = BK * ROWS / 2;
-    for (int c = tid; c < CHUNKS; c += NTHREADS) {
-      int kk = c / (ROWS / 2), cc = c % (ROWS / 2);
-      int k = k0 + kk, row = row0 + cc * 2;
-      double* dst = s + kk * PITCH + cc * 2;
-      bool kok = k < K;
-      const double* src = g + (kok ? (long long)k * ld : 0) + (row < nrows ? row : 0);
-      int nb = kok ? max(0, min(2, nrows - row)) * 8 : 0;
+    kstep = KMAJOR ? BK : (long long)BK * ld;
+  }
+  // copy the slab of k-tile kt of operand base `g` into stage `s`
+  __device__ __forceinline__ void issue(double* s, const double* __restrict__ g, int kt, int K) const {
+    const int k0 = kt * BK;
+    const double* gk = g + (long long)kt * kstep;
+#pragma unroll
+    for (int q = 0; q < NCH; q++) {
+      if (NCH * NTHREADS != CHUNKS && bytes[q] == 0 && threadIdx.x + q * NTHREADS >= CHUNKS) continue;
+      const int krem = K - (k0 + kofs[q]);                   // k values left from this chunk's first k
+      int nb;
+      if (KMAJOR) nb = krem >= 2 ? bytes[q] : (krem == 1 ? min(bytes[q], 8) : 0);
+      else nb = krem >= 1 ? bytes[q] : 0;
+      const double* src = nb > 0 ? gk + goff[q] : g;
+      double* dst = s + soff[q];
       if (AL16) {
         cp_async16(dst, src, nb);
       } else {
@@ -85,7 +103,7 @@ __device__ __forceinline__ void load_tile(double* s, const double* __restrict__ 
       }
     }
   }
-}
+};
 
 template <int BM, int BN, int BK, int WM, int WN, int STAGES, bool AKM, bool BKM, bool AL16>
 __global__ void __launch_bounds__(WM* WN * 32) dgemm_kernel(const GemmParams p) {
@@ -117,38 +135,48 @@ __global__ void __launch_bounds__(WM* WN * 32) dgemm_kernel(const GemmParams p) 
 #pragma unroll
     for (int j = 0; j < NT; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-  auto issue = [&](int li) {   // li = local iteration index
-    if (li < nit) {
-      int it = it_begin + li;
-      int kb = it / ktiles, kt = it - kb * ktiles;
-      int st = li % STAGES;
-      load_tile<BM, BK, NTHREADS, AKM, AL16>(sA + st * A_STAGE, Ab + (long long)kb * p.sAk, p.lda, m0, p.M, kt * BK, p.K, tid);
-      load_tile<BN, BK, NTHREADS, BKM, AL16>(sB + st * B_STAGE, Bb + (long long)kb * p.sBk, p.ldb, n0, p.N, kt * BK, p.K, tid);
+  TileLoader<BM, BK, NTHREADS, AKM, AL16> ldA;
+  TileLoader<BN, BK, NTHREADS, BKM, AL16> ldB;
+  ldA.init(p.lda, m0, p.M, tid);
+  ldB.init(p.ldb, n0, p.N, tid);
+  // (kb, kt) of the next slab to fetch, advanced incrementally (no division in the loop)
+  int f_kb = it_begin / ktiles, f_kt = it_begin - f_kb * ktiles, f_li = 0;
+  auto issue = [&]() {
+    if (f_li < nit) {
+      const int st = f_li % STAGES;
+      ldA.issue(sA + st * A_STAGE, Ab + (long long)f_kb * p.sAk, f_kt, p.K);
+      ldB.issue(sB + st * B_STAGE, Bb + (long long)f_kb * p.sBk, f_kt, p.K);
+      if (++f_kt == ktiles) { f_kt = 0; f_kb++; }
     }
+    f_li++;
     cp_async_commit();
   };
 
 #pragma unroll
-  for (int s = 0; s < STAGES - 1; s++) issue(s);
+  for (int s = 0; s < STAGES - 1; s++) issue();
 
   for (int li = 0; li < nit; li++) {
     cp_async_wait<STAGES - 2>();
     __syncthreads();
-    issue(li + STAGES - 1);
+    // the two warps that share an SM sub-partition (w and w + 4) fetch at different times, so that one of them is always
+    // issuing DMMAs while the other does its cp.async address work
+    const bool fetch_first = ((warp >> 2) & 1) == 0;
+    if (fetch_first) issue();
     const double* a_s = sA + (li % STAGES) * A_STAGE;
     const double* b_s = sB + (li % STAGES) * B_STAGE;
-#pragma unroll
-    for (int kb8 = 0; kb8 < BK / 8; kb8++) {
-      double af[MT][2], bf[NT][2];
+    // fragments of k-block kb8 (8 k = two k4 steps h: k = 2t + h), double-buffered in registers so that the loads of
+    // block kb8 + 1 are in flight while the 2 * MT * NT DMMAs of block kb8 issue
+    double af[2][MT][2], bf[2][NT][2];
+    auto load_frags = [&](int buf, int kb8) {
 #pragma unroll
       for (int i = 0; i < MT; i++) {
         int r = wm * WTM + i * 8 + g;
         if (AKM) {
           double2 v = *reinterpret_cast<const double2*>(a_s + (kb8 * BM + r) * 8 + 2 * t);
-          af[i][0] = v.x; af[i][1] = v.y;
+          af[buf][i][0] = v.x; af[buf][i][1] = v.y;
         } else {
-          af[i][0] = a_s[(kb8 * 8 + 2 * t) * (BM + 2) + r];
-          af[i][1] = a_s[(kb8 * 8 + 2 * t + 1) * (BM + 2) + r];
+          af[buf][i][0] = a_s[(kb8 * 8 + 2 * t) * (BM + 2) + r];
+          af[buf][i][1] = a_s[(kb8 * 8 + 2 * t + 1) * (BM + 2) + r];
         }
       }
 #pragma unroll
@@ -156,18 +184,24 @@ __global__ void __launch_bounds__(WM* WN * 32) dgemm_kernel(const GemmParams p) 
         int r = wn * WTN + j * 8 + g;
         if (BKM) {
           double2 v = *reinterpret_cast<const double2*>(b_s + (kb8 * BN + r) * 8 + 2 * t);
-          bf[j][0] = v.x; bf[j][1] = v.y;
+          bf[buf][j][0] = v.x; bf[buf][j][1] = v.y;
         } else {
-          bf[j][0] = b_s[(kb8 * 8 + 2 * t) * (BN + 2) + r];
-          bf[j][1] = b_s[(kb8 * 8 + 2 * t + 1) * (BN + 2) + r];
+          bf[buf][j][0] = b_s[(kb8 * 8 + 2 * t) * (BN + 2) + r];
+          bf[buf][j][1] = b_s[(kb8 * 8 + 2 * t + 1) * (BN + 2) + r];
         }
       }
+    };
+    load_frags(0, 0);
+#pragma unroll
+    for (int kb8 = 0; kb8 < BK / 8; kb8++) {
+      if (kb8 + 1 < BK / 8) load_frags((kb8 + 1) & 1, kb8 + 1);
 #pragma unroll
       for (int h = 0; h < 2; h++)
 #pragma unroll
         for (int i = 0; i < MT; i++)
 #pragma unroll
-          for (int j = 0; j < NT; j++) dmma884(acc[i][j][0], acc[i][j][1], af[i][h], bf[j][h]);
+          for (int j = 0; j < NT; j++) dmma884(acc[i][j][0], acc[i][j][1], af[kb8 & 1][i][h], bf[kb8 & 1][j][h]);
+      if (kb8 == 0 && !fetch_first) issue();
     }
   }
   cp_async_wait<0>();

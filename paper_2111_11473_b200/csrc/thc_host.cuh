@@ -6,6 +6,7 @@
 #include <stdint.h>
 #include <stdio.h>
 #include <algorithm>
+#include <cmath>
 #include <string>
 #include <vector>
 #include "../../include/thc.h"
@@ -144,17 +145,26 @@ struct Ctx {
   // ---- GEMM ----------------------------------------------------------------------------------------------------
   void gemm(const Gemm& g) {
     if (g.M <= 0 || g.N <= 0 || g.nbatch <= 0) return;
-    const i64 tb = (i64)((g.M + 127) / 128) * ((g.N + 127) / 128) * g.nbatch;
-    const bool big = (g.M > 64 && g.N > 64 && tb * 2 >= h->sms);
+    // Tile shape and split-K factor: minimise  waves x (k-iterations per CTA + fixed cost) x tile area / tile rate  over
+    // {128x128 (1 CTA/SM), 64x64 (3 CTAs/SM)} x splits; a split-K pass adds a partial-tile write and a reduction.
+    const i64 kiters = (i64)g.nkb * ((g.K + 15) / 16);
+    bool big = false; int splits = 1; double best = 1e300;
+    for (int cfg = 0; cfg < 2; cfg++) {
+      const int T = cfg == 0 ? 128 : 64;
+      if (cfg == 0 && (g.M <= 64 || g.N <= 64)) continue;
+      const i64 tmn = (i64)((g.M + T - 1) / T) * ((g.N + T - 1) / T) * g.nbatch;
+      const double slots = (double)h->sms * (cfg == 0 ? 1 : 3);
+      const double rate = cfg == 0 ? 1.0 : 0.72 / 3.0;           // per-CTA DMMA rate relative to a 128x128 CTA owning an SM
+      const int smax = (int)std::max<i64>(1, std::min<i64>(64, kiters / 8));
+      for (int sp = 1; sp <= smax; sp++) {
+        const double waves = std::ceil((double)tmn * sp / slots);
+        double t = waves * ((double)kiters / sp + 6.0) * T * T / rate;
+        if (sp > 1) t += 0.025 * sp * (double)g.M * g.N * g.nbatch;     // partial-tile write + reduction at ~5 TB/s, same units
+        if (t < best * (sp > 1 ? 0.97 : 1.0)) { best = t; big = cfg == 0; splits = sp; }
+      }
+    }
     const int BMN = big ? 128 : 64;
     const i64 tiles_mn = (i64)((g.M + BMN - 1) / BMN) * ((g.N + BMN - 1) / BMN);
-    const i64 tiles = tiles_mn * g.nbatch;
-    const i64 kiters = (i64)g.nkb * ((g.K + 15) / 16);
-    int splits = 1;
-    if (tiles < h->sms && kiters >= 16) {
-      splits = (int)std::min<i64>(std::min<i64>((2 * h->sms + tiles - 1) / tiles, kiters / 8), 64);
-      if (splits < 1) splits = 1;
-    }
     const i64 per = (i64)g.nbatch * g.M * g.N;
     if (splits > 1) splitk_need = std::max(splitk_need, per * splits);
     if (dry || !ok()) return;
