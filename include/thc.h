@@ -50,8 +50,23 @@ typedef enum {
   THC_ERR_OVERFLOW = -2,      /* a buffer size does not fit in 63 bits                          */
   THC_ERR_NO_MEMORY = -3,     /* workspace too small / cudaMalloc failed                        */
   THC_ERR_CUDA = -4,          /* a CUDA call or kernel launch failed (see thc_last_cuda_error)  */
-  THC_ERR_NO_DEVICE = -5      /* no sm_100 device visible                                       */
+  THC_ERR_NO_DEVICE = -5,     /* no sm_100 device visible                                       */
+  THC_ERR_PROVIDER = -6       /* a thc_bvv_provider callback returned non-zero                   */
 } thc_status;
+
+/* Where the vv Cholesky blocks B_vv[NL][v][v] live (PAPER.md l.191-195 keeps the 3-index arrays off the GPU and
+ * streams them; at the paper-scale config B_vv is ~304 GB and can never be resident):
+ *   THC_BVV_DEVICE    B_vv is a device pointer to the whole array (default).
+ *   THC_BVV_HOST      B_vv is a HOST pointer to the whole array (pinned memory makes the copies overlap); the library
+ *                     copies one L-block at a time into a double buffer on its own copy stream, overlapped with the
+ *                     GEMMs of the previous block.
+ *   THC_BVV_PROVIDER  B_vv points to a thc_bvv_provider; for every L-block the library calls
+ *                     fill(ctx, L0, nl, dst, stream), which must enqueue on `stream` (a cudaStream_t) work that writes
+ *                     B_vv[L0 .. L0+nl) as dst[nl][v][v] (device memory) and return 0.  Called in increasing L0, from
+ *                     the calling thread, before thc_residual returns.                                            */
+typedef enum { THC_BVV_DEVICE = 0, THC_BVV_HOST = 1, THC_BVV_PROVIDER = 2 } thc_bvv_mode;
+typedef int (*thc_bvv_fill_fn)(void* ctx, int64_t L0, int64_t nl, double* dst_device, void* cuda_stream);
+typedef struct { thc_bvv_fill_fn fill; void* ctx; } thc_bvv_provider;
 
 /* Bits of thc_options.term_mask (terms to evaluate; 0 means all). */
 enum { THC_TERM_S1 = 1, THC_TERM_S2 = 2, THC_TERM_S3 = 4, THC_TERM_S6 = 8, THC_TERM_S7 = 16, THC_TERM_S9 = 32,
@@ -65,6 +80,8 @@ typedef struct {
   int64_t workspace_bytes_max; /* cap for the auto block-size choice (0 = 75 % of free device memory)       */
   int32_t term_mask;        /* THC_TERM_* bits, 0 = all                                                     */
   int32_t device;           /* CUDA device ordinal, -1 = current device                                     */
+  int32_t bvv_mode;         /* thc_bvv_mode: what the B_vv argument of thc_residual[_terms] is                  */
+  int32_t reserved;         /* must be 0                                                                    */
 } thc_options;
 
 /* Create a handle for one problem shape.  (o, v, NL, NP, NX) as in BASELINE.json / PAPER.md l.47-54

@@ -51,7 +51,24 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 class _Options(ctypes.Structure):
     _fields_ = [("bL", ctypes.c_int64), ("bP7", ctypes.c_int64), ("bX", ctypes.c_int64), ("bI", ctypes.c_int64),
-                ("workspace_bytes_max", ctypes.c_int64), ("term_mask", ctypes.c_int32), ("device", ctypes.c_int32)]
+                ("workspace_bytes_max", ctypes.c_int64), ("term_mask", ctypes.c_int32), ("device", ctypes.c_int32),
+                ("bvv_mode", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+
+
+BVV_MODES = dict(device=0, host=1, provider=2)
+_FILL_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_int64, ctypes.c_int64, ctypes.c_void_p, ctypes.c_void_p)
+
+
+class _BvvProvider(ctypes.Structure):
+    _fields_ = [("fill", _FILL_FN), ("ctx", ctypes.c_void_p)]
+
+
+class _DevView:
+    """Zero-copy torch view of device memory the library owns (handed to a B_vv provider callback)."""
+
+    def __init__(self, ptr, shape):
+        self.__cuda_array_interface__ = dict(data=(int(ptr), False), shape=tuple(int(x) for x in shape), typestr="<f8",
+                                             version=2, strides=None)
 
 
 _lib = None
@@ -128,13 +145,14 @@ class Thc:
     """One problem shape (thc_setup ... thc_destroy).  Methods mirror the C entry points."""
 
     def __init__(self, o, v, NL, NP, NX, *, bL=0, bP7=0, bX=0, bI=0, workspace_bytes_max=0, term_mask=0,
-                 device=-1, torch_workspace=True):
+                 device=-1, torch_workspace=True, bvv_mode="device"):
         import torch
         if not torch.cuda.is_available():
             raise ThcError("no CUDA device: the THC residual has no CPU path")
         self.o, self.v, self.NL, self.NP, self.NX = o, v, NL, NP, NX
         self._h = ctypes.c_void_p()
-        opt = _Options(bL, bP7, bX, bI, workspace_bytes_max, term_mask, device)
+        self.bvv_mode = bvv_mode
+        opt = _Options(bL, bP7, bX, bI, workspace_bytes_max, term_mask, device, BVV_MODES[bvv_mode], 0)
         _check(lib().thc_setup(ctypes.byref(self._h), o, v, NL, NP, NX, ctypes.byref(opt)))
         self._ws = None
         self._torch_ws = torch_workspace
@@ -180,10 +198,34 @@ class Thc:
     def algorithmic_flops(self):
         return float(lib().thc_algorithmic_flops(self._h))
 
+    def _bvv_ptr(self, B_vv, conv):
+        """B_vv argument per thc_bvv_mode: device tensor, host tensor, or a callable fill(L0, nl, dst) that writes
+        B_vv[L0:L0+nl] into the device tensor dst[nl, v, v] on torch's current stream."""
+        import torch
+        v, NL = self.v, self.NL
+        if self.bvv_mode == "device":
+            return conv(B_vv, "B_vv", NL * v * v)
+        if self.bvv_mode == "host":
+            return _host_ptr(B_vv, "B_vv", NL * v * v)
+        if not callable(B_vv):
+            raise ThcError("B_vv: bvv_mode='provider' needs a callable fill(L0, nl, dst)")
+
+        def _fill(ctx, L0, nl, dst, stream):
+            try:
+                with torch.cuda.stream(torch.cuda.ExternalStream(stream or 0, device=self._device)):
+                    B_vv(int(L0), int(nl), torch.as_tensor(_DevView(dst, (nl, v, v)), device=self._device))
+                return 0
+            except Exception as exc:            # never let an exception cross the C ABI
+                self._provider_error = exc
+                return 1
+
+        self._provider = _BvvProvider(_FILL_FN(_fill), None)     # kept alive for the duration of the call
+        return ctypes.cast(ctypes.pointer(self._provider), ctypes.c_void_p)
+
     def _in_ptrs(self, Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps, conv):
         o, v, NL, NP, NX = self.o, self.v, self.NL, self.NP, self.NX
         return [conv(Xo, "Xo", o * NP), conv(Xv, "Xv", v * NP), conv(Z, "Z", NP * NP),
-                conv(B_ov, "B_ov", NL * o * v), conv(B_oo, "B_oo", NL * o * o), conv(B_vv, "B_vv", NL * v * v),
+                conv(B_ov, "B_ov", NL * o * v), conv(B_oo, "B_oo", NL * o * o), self._bvv_ptr(B_vv, conv),
                 conv(Y, "Y", (o + v) * NX), conv(V, "V", NX * NX), conv(eps, "eps", o + v)]
 
     # ---- entry points ---------------------------------------------------------------------------------------

@@ -31,6 +31,11 @@ struct thc_handle {
   struct TripleList { int64_t nPp, NPp; thc::TripleItem* dev; int n; };
   std::vector<TripleList> tp_lists;
   void* encode_tiled;                // cuTensorMapEncodeTiled, resolved through the runtime (no -lcuda link)
+  // B_vv streaming (THC_BVV_HOST): copy stream and double-buffer events, created on first use
+  int bvv_mode;
+  cudaStream_t copy_stream;
+  cudaEvent_t ev_loaded[2], ev_free[2], ev_start;
+  bool copy_ready;
   // per-class kernel timing (thc_profile_begin / thc_profile_end): CUDA events recorded on `stream` around every
   // launch of a class whose bit is set in prof_mask
   int prof_mask;
@@ -154,10 +159,13 @@ struct Ctx {
       if (cfg == 0 && (g.M <= 64 || g.N <= 64)) continue;
       const i64 tmn = (i64)((g.M + T - 1) / T) * ((g.N + T - 1) / T) * g.nbatch;
       const double slots = (double)h->sms * (cfg == 0 ? 1 : 3);
-      const double rate = cfg == 0 ? 1.0 : 0.72 / 3.0;           // per-CTA DMMA rate relative to a 128x128 CTA owning an SM
       const int smax = (int)std::max<i64>(1, std::min<i64>(64, kiters / 8));
       for (int sp = 1; sp <= smax; sp++) {
         const double waves = std::ceil((double)tmn * sp / slots);
+        // per-CTA DMMA rate relative to a 128x128 CTA that owns an SM: a lone 64x64 CTA (one warp per sub-partition)
+        // reaches ~0.5, three of them share ~0.75 of the pipe
+        const double conc = std::min(3.0, std::ceil((double)tmn * sp / h->sms));
+        const double rate = cfg == 0 ? 1.0 : std::min(0.5, 0.75 / conc);
         double t = waves * ((double)kiters / sp + 6.0) * T * T / rate;
         if (sp > 1) t += 0.025 * sp * (double)g.M * g.N * g.nbatch;     // partial-tile write + reduction at ~5 TB/s, same units
         if (t < best * (sp > 1 ? 0.97 : 1.0)) { best = t; big = cfg == 0; splits = sp; }
@@ -302,6 +310,36 @@ struct Ctx {
     launched();
     prof_stop(2);
   }
+  // ---- B_vv streaming (THC_BVV_HOST / THC_BVV_PROVIDER) ------------------------------------------------------------
+  void bvv_begin() {
+    if (!ok() || h->bvv_mode != THC_BVV_HOST) return;
+    if (!h->copy_ready) {
+      check(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
+      for (int k = 0; k < 2; k++) {
+        check(cudaEventCreateWithFlags(&h->ev_loaded[k], cudaEventDisableTiming));
+        check(cudaEventCreateWithFlags(&h->ev_free[k], cudaEventDisableTiming));
+      }
+      check(cudaEventCreateWithFlags(&h->ev_start, cudaEventDisableTiming));
+      h->copy_ready = ok();
+    }
+    // the copy stream may not touch the double buffer before earlier work on the compute stream has finished with it
+    check(cudaEventRecord(h->ev_start, h->stream));
+    check(cudaStreamWaitEvent(h->copy_stream, h->ev_start, 0));
+  }
+  void bvv_copy(double* dst, const double* host, i64 L0, i64 nl, i64 v, i64 blk) {
+    if (!ok()) return;
+    if (blk >= 2) check(cudaStreamWaitEvent(h->copy_stream, h->ev_free[blk & 1], 0));
+    check(cudaMemcpyAsync(dst, host + L0 * v * v, (size_t)(nl * v * v) * 8, cudaMemcpyHostToDevice, h->copy_stream));
+    check(cudaEventRecord(h->ev_loaded[blk & 1], h->copy_stream));
+  }
+  void bvv_wait_loaded(i64 blk) { if (ok()) check(cudaStreamWaitEvent(h->stream, h->ev_loaded[blk & 1], 0)); }
+  void bvv_release(i64 blk) { if (ok()) check(cudaEventRecord(h->ev_free[blk & 1], h->stream)); }
+  void bvv_provide(const thc_bvv_provider* pr, i64 L0, i64 nl, double* dst) {
+    if (!ok()) return;
+    if (!pr || !pr->fill) { status = THC_ERR_INVALID_ARG; return; }
+    if (pr->fill(pr->ctx, L0, nl, dst, (void*)h->stream) != 0) status = THC_ERR_PROVIDER;
+  }
+
   // TMA descriptor over a [d2][d1][d0] FP64 array (d0 contiguous), box 16 x 16 x 1, 128-byte swizzle.
   bool make_map3(CUtensorMap* m, const double* base, i64 d0, i64 d1, i64 d2) {
     typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,

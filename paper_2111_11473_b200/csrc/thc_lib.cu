@@ -75,9 +75,30 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out) {
   // ---- L-block loop: Alg.1 + Alg.3 (H1-H4) and Alg.2 + Alg.8 (H5-H6) fused over the Cholesky index (l.238) ---------
   const bool need_ladder = do_s1 || do_s3;
   const bool need_ring = do_s2 || do_s9;
-  for (i64 L0 = 0; L0 < NL; L0 += h->bL) {
+  // B_vv source: resident (device pointer), or streamed one L-block at a time into a double buffer (l.191-195)
+  const bool streamed = h->bvv_mode != THC_BVV_DEVICE && need_ladder;
+  double* bvv_buf[2] = {nullptr, nullptr};
+  if (streamed) { bvv_buf[0] = ar.alloc(h->bL * v * v); bvv_buf[1] = ar.alloc(h->bL * v * v); }
+  if (streamed && !c.dry) c.bvv_begin();
+  if (streamed && !c.dry && h->bvv_mode == THC_BVV_HOST)
+    c.bvv_copy(bvv_buf[0], in.B_vv, 0, std::min<i64>(h->bL, NL), v, 0);
+  i64 blk = 0;
+  for (i64 L0 = 0; L0 < NL; L0 += h->bL, blk++) {
     const i64 nl = std::min<i64>(h->bL, NL - L0);
     const i64 m0 = ar.mark();
+    const double* bvv = in.B_vv + L0 * v * v;
+    if (streamed) {
+      bvv = bvv_buf[blk & 1];
+      if (!c.dry) {
+        if (h->bvv_mode == THC_BVV_HOST) {
+          const i64 L1 = L0 + h->bL;                 // prefetch the next block while this one is consumed
+          if (L1 < NL) c.bvv_copy(bvv_buf[(blk + 1) & 1], in.B_vv, L1, std::min<i64>(h->bL, NL - L1), v, blk + 1);
+          c.bvv_wait_loaded(blk);
+        } else {
+          c.bvv_provide(reinterpret_cast<const thc_bvv_provider*>(in.B_vv), L0, nl, bvv_buf[blk & 1]);
+        }
+      }
+    }
     if (need_ladder) {
       double* T1T = ar.alloc(NP * nl * o);
       double* T2T = ar.alloc(NP * nl * v);
@@ -86,7 +107,8 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out) {
       c.gemm(Gemm(XoT, o, 'K', in.B_oo + L0 * o * o, o, 'K', T1T, nl * o, NP, nl * o, o));
       c.gemm(Gemm(T1T, nl * o, 'K', XoT, o, 'K', Mo, NP, NP, NP, o).batch(nl, o, 0, NP2));
       // H2: same with the vv block                                                                  (Alg.1 lines 10-11)
-      c.gemm(Gemm(XvT, v, 'K', in.B_vv + L0 * v * v, v, 'K', T2T, nl * v, NP, nl * v, v));
+      c.gemm(Gemm(XvT, v, 'K', bvv, v, 'K', T2T, nl * v, NP, nl * v, v));
+      if (streamed && !c.dry && h->bvv_mode == THC_BVV_HOST) c.bvv_release(blk);
       c.gemm(Gemm(T2T, nl * v, 'K', XvT, v, 'K', Mv, NP, NP, NP, v).batch(nl, v, 0, NP2));
       // H3: C^l = v .* Mo^l - o .* Mv^l (in place over Mo);  C3 += Mo^l .* Mv^l                   (Alg.1 l.8,12,13; Alg.3 l.7)
       c.combine(Mo, Mv, omat, vmat, C3, NP2, nl);
@@ -317,7 +339,10 @@ i64 input_doubles(const thc_handle* h, i64 sizes[9]) {
   const i64 o = h->o, v = h->v, NL = h->NL, NP = h->NP, NX = h->NX;
   const i64 s[9] = {o * NP, v * NP, NP * NP, NL * o * v, NL * o * o, NL * v * v, (o + v) * NX, NX * NX, o + v};
   i64 tot = 0;
-  for (int k = 0; k < 9; k++) { sizes[k] = s[k]; tot += (s[k] * 8 + 255) / 256 * 256; }
+  for (int k = 0; k < 9; k++) {
+    sizes[k] = (k == 5 && h->bvv_mode != THC_BVV_DEVICE) ? 0 : s[k];     // a streamed B_vv is never staged as a whole
+    tot += (sizes[k] * 8 + 255) / 256 * 256;
+  }
   return tot;   // bytes
 }
 i64 need_device(thc_handle* h) { return std::max<i64>(dry_residual(h).total(), dry_energy(h).total()); }
@@ -399,6 +424,7 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
   if (!hp) return THC_ERR_INVALID_ARG;
   *hp = nullptr;
   if (o <= 0 || v <= 0 || NL <= 0 || NP <= 0 || NX <= 0) return THC_ERR_INVALID_ARG;
+  if (opt && (opt->bvv_mode < 0 || opt->bvv_mode > 2 || opt->reserved != 0)) return THC_ERR_INVALID_ARG;
   if (opt && (opt->bL < 0 || opt->bP7 < 0 || opt->bX < 0 || opt->bI < 0 || opt->workspace_bytes_max < 0)) return THC_ERR_INVALID_ARG;
   const int64_t lim = (int64_t)1 << 31;
   if (o >= lim || v >= lim || NL >= lim || NP >= lim || NX >= lim) return THC_ERR_OVERFLOW;
@@ -424,6 +450,7 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
   h->stream = nullptr; h->ws = nullptr; h->ws_bytes = 0; h->ws_owned = false;
   h->launches = 0; h->last_cuda = 0; h->smem_configured = false;
   h->prof_mask = 0; h->prof_used = 0; h->encode_tiled = nullptr;
+  h->bvv_mode = opt ? opt->bvv_mode : THC_BVV_DEVICE; h->copy_stream = nullptr; h->copy_ready = false;
 
   // block sizes: defaults, then shrink until the plan fits the cap
   h->bL = std::min<int64_t>(NL, (opt && opt->bL) ? opt->bL : 32);
@@ -458,12 +485,18 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
 
 int thc_destroy(thc_handle* h) {
   if (!h) return THC_ERR_INVALID_ARG;
-  if ((h->ws && h->ws_owned) || !h->prof_events.empty() || !h->tp_lists.empty()) {
+  if ((h->ws && h->ws_owned) || !h->prof_events.empty() || !h->tp_lists.empty() || h->copy_ready) {
     DeviceGuard g(h->device);
     cudaStreamSynchronize(h->stream);
     if (h->ws && h->ws_owned) cudaFree(h->ws);
     for (cudaEvent_t e : h->prof_events) cudaEventDestroy(e);
     for (auto& l : h->tp_lists) cudaFree(l.dev);
+    if (h->copy_ready) {
+      cudaStreamSynchronize(h->copy_stream);
+      for (int k = 0; k < 2; k++) { cudaEventDestroy(h->ev_loaded[k]); cudaEventDestroy(h->ev_free[k]); }
+      cudaEventDestroy(h->ev_start);
+      cudaStreamDestroy(h->copy_stream);
+    }
   }
   delete h;
   return THC_OK;
@@ -589,6 +622,7 @@ int thc_residual_host(thc_handle* h, const double* Xo, const double* Xv, const d
   double* dev[9];
   for (int k = 0; k < 9; k++) {
     dev[k] = reinterpret_cast<double*>(p);
+    if (sz[k] == 0) { dev[k] = const_cast<double*>(src[k]); continue; }
     cudaError_t e = cudaMemcpyAsync(dev[k], src[k], (size_t)sz[k] * 8, cudaMemcpyHostToDevice, h->stream);
     if (e != cudaSuccess) { h->last_cuda = (int)e; return THC_ERR_CUDA; }
     p += (sz[k] * 8 + 255) / 256 * 256;
@@ -686,6 +720,7 @@ const char* thc_strerror(int status) {
     case THC_ERR_NO_MEMORY: return "workspace too small or device allocation failed";
     case THC_ERR_CUDA: return "CUDA error (see thc_last_cuda_error)";
     case THC_ERR_NO_DEVICE: return "no sm_100 CUDA device";
+    case THC_ERR_PROVIDER: return "B_vv provider callback failed";
     default: return "unknown status";
   }
 }

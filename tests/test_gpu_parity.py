@@ -113,3 +113,34 @@ def test_host_entry_matches_oracle(oracle_cfg):
     assert _relerr(R.numpy(), ref["R"]) <= RTOL
     assert abs(E - ref["E"]) <= ETOL
     h.close()
+
+
+@pytest.mark.parametrize("mode", ["host", "provider"])
+def test_streamed_bvv_matches_resident(mode):
+    """B_vv streamed in L-blocks (pinned host memory, or a provider callback that fills device blocks on demand;
+    PAPER.md l.191-195, BASELINE config 4) must give bit-identical results to the resident path."""
+    import torch
+    import paper_2111_11473_b200 as thc
+    x = small_inputs(6, 14, 21, 40, 52, seed=3, zmul=30.0)
+    ref = oracle_eval(x)
+    d = _to_dev(x)
+    h0 = thc.thc_setup(x.o, x.v, x.NL, x.NP, x.NX, bL=4)
+    R0 = h0.thc_residual(*d).cpu().numpy()
+    h0.close()
+    h = thc.thc_setup(x.o, x.v, x.NL, x.NP, x.NX, bL=4, bvv_mode=mode)
+    calls = []
+    if mode == "host":
+        bvv = torch.from_numpy(np.ascontiguousarray(x.B_vv)).pin_memory()
+    else:
+        def bvv(L0, nl, dst):
+            calls.append((L0, nl))
+            dst.copy_(d[5][L0:L0 + nl])
+    args = list(d)
+    args[5] = bvv
+    for _ in range(2):                      # twice: the double buffer must be reusable across calls
+        R = h.thc_residual(*args).cpu().numpy()
+        assert np.array_equal(R, R0)
+    assert _relerr(R, ref["R"]) <= RTOL
+    if mode == "provider":
+        assert calls[:3] == [(0, 4), (4, 4), (8, 4)] and calls[5] == (20, 1)
+    h.close()
