@@ -51,7 +51,9 @@ class RowOracle:
         Xo_jQ Xv_bQ spelled out.  tidx is a 4-letter string (i, a, j, b positions); P, Q are reserved letters."""
         i, a, j, b = tidx
         spec = f"{i}P,{a}P,PQ,{j}Q,{b}Q,{oidx}->{out}"
-        return np.einsum(spec, self.Xo, self.Xv, self.Z, self.Xo, self.Xv, other, optimize=True)
+        # the explicit memory limit only lets the path search form intermediates larger than its operands (e.g. [L,P,Q]);
+        # the default limit would force a single 5-operand step of naive scaling
+        return np.einsum(spec, self.Xo, self.Xv, self.Z, self.Xo, self.Xv, other, optimize=("optimal", 2 ** 34))
 
     def _u(self, x):
         """(u x)_kc = sum_ia (2 t_ik^ac - t_ik^ca) x_ia,  u[i,a,k,c] = 2 t[i,a,k,c] - t[i,c,k,a]."""
@@ -150,7 +152,8 @@ class RowOracle:
 
     def _thc_exchange(self, x):
         """y_ld = sum_kc x_kc <kd|lc>."""
-        return np.einsum("kc,kI,dI,IJ,lJ,cJ->ld", x, self.Yo, self.Yv, self.V, self.Yo, self.Yv, optimize=True)
+        return np.einsum("kc,kI,dI,IJ,lJ,cJ->ld", x, self.Yo, self.Yv, self.V, self.Yo, self.Yv,
+                         optimize=("optimal", 2 ** 34))
 
     def _row_s7(self, w, P):
         """Eq.35 l.261 corrected (R2, R3): 1/2 sum_klcd [ u_ik^ac (2<kc|ld> - <kd|lc>) u_jl^bd + t_ik^ca <kd|lc> t_jl^db ]."""
@@ -176,11 +179,11 @@ class RowOracle:
             # Eq.32: <kc|ld> = sum_IJ Yo_kI Yv_cI V_IJ Yo_lJ Yv_dJ
             th = np.einsum("cjd,cI,dJ->jIJ", theta, Yv_c, self.Yv, optimize=True)
             ta = np.einsum("klb,kI,lJ->bIJ", tau, Yo_c, self.Yo, optimize=True)
-            r += np.einsum("IJ,jIJ,bIJ->jb", V_c, th, ta, optimize=True)
+            r += (V_c[None] * th).reshape(self.o, -1) @ ta.reshape(self.v, -1).T          # sum_IJ V_IJ th[j,I,J] ta[b,I,J]
             # Eq.33: <lc|kd> = sum_IJ Yo_lI Yv_cI V_IJ Yo_kJ Yv_dJ
             ph = np.einsum("ckb,cI,kJ->bIJ", theta, Yv_c, self.Yo, optimize=True)
             ps = np.einsum("ljd,lI,dJ->jIJ", tau, Yo_c, self.Yv, optimize=True)
-            r += np.einsum("IJ,bIJ,jIJ->jb", V_c, ph, ps, optimize=True)
+            r += (V_c[None] * ps).reshape(self.o, -1) @ ph.reshape(self.v, -1).T          # sum_IJ V_IJ ps[j,I,J] ph[b,I,J]
         return r
 
     # ---- energy (reading R7): E = sum_ijab (2 t_ij^ab - t_ij^ba)(ia|jb), Cholesky ERIs, in extended precision ------------

@@ -1,0 +1,68 @@
+"""Parity of the CUDA path against the T2 sampled-row oracle (oracle/rows.py) at sizes the dense oracle cannot hold.
+
+Config 2 (o=60, v=340, NL=1200, NP=1000, NX=2000) runs by default, in the launch configuration bench.py times; config 3
+is opt-in (THC_BIG_TESTS=1: ~20 GB of inputs and minutes of CPU per row).  Inputs are drawn on the device by
+thc_synth.device and the very same tensors are copied to the host for the oracle.  Tolerances as in test_gpu_parity.py:
+1e-10 relative to each term's own maximum over the sampled rows, 1e-9 E_h on the energy.
+"""
+import os
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TERMS = ("s1", "s2", "s3", "s6", "s7", "s9")
+NAMES = ("Xo", "Xv", "Z", "B_ov", "B_oo", "B_vv", "Y", "V", "eps")
+
+
+def _run(cfg, rows, rows_s6, lblock):
+    import torch
+    import paper_2111_11473_b200 as thc
+    from thc_synth import CONFIGS
+    from thc_synth.device import make_config_device
+    from oracle.rows import RowOracle
+
+    c = CONFIGS[cfg]
+    d = make_config_device(cfg)
+    h = thc.thc_setup(c["o"], c["v"], c["NL"], c["NP"], c["NX"])
+    args = [d[n] for n in NAMES]
+    res = h.thc_residual_terms(*args)
+    E = h.thc_energy(d["Xo"], d["Xv"], d["Z"], d["B_ov"])
+    torch.cuda.synchronize()
+    got = {k: res[k][list(rows)].cpu().numpy() for k in TERMS + ("R",)}
+    xi_oo, xi_vv = res["xi_oo"].cpu().numpy(), res["xi_vv"].cpu().numpy()
+    sym = float((res["R"] - res["R"].T).abs().max() / res["R"].abs().max())
+    h.close()
+    del res
+    host = {n: d[n].cpu().numpy() for n in NAMES}
+    del d, args
+    torch.cuda.empty_cache()
+
+    ro = RowOracle(*[host[n] for n in NAMES], lblock=lblock)
+    errs = {"R_symmetry": sym}
+    rxo, rxv = ro.xi()
+    errs["xi_oo"] = np.abs(xi_oo - rxo).max() / np.abs(rxo).max()
+    errs["xi_vv"] = np.abs(xi_vv - rxv).max() / np.abs(rxv).max()
+    errs["E_abs"] = abs(E - ro.energy())
+    ref = {k: [] for k in TERMS}
+    for n, P in enumerate(rows):
+        terms = TERMS if P in rows_s6 else tuple(k for k in TERMS if k != "s6")
+        r = ro.row(P, terms=terms)
+        for k in terms:
+            ref[k].append((n, r[k]))
+    for k in TERMS:
+        scale = max(np.abs(r).max() for _, r in ref[k])
+        errs[k] = max(np.abs(got[k][n] - r).max() for n, r in ref[k]) / scale
+    bad = {k: e for k, e in errs.items() if e > (1e-9 if k == "E_abs" else 1e-10)}
+    assert not bad, f"parity failures {bad} (all: {errs})"
+    print(f"config {cfg} sampled-row parity: {errs}")
+
+
+def test_config2_sampled_rows():
+    _run(2, rows=(3, 777), rows_s6=(3,), lblock=16)
+
+
+@pytest.mark.skipif(not os.environ.get("THC_BIG_TESTS"), reason="set THC_BIG_TESTS=1 (config 3: ~20 GB, minutes of CPU per row)")
+def test_config3_sampled_rows():
+    _run(3, rows=(1234,), rows_s6=(1234,), lblock=8)

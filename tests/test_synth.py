@@ -42,3 +42,18 @@ def test_structure_and_distributions():
 def test_configs_match_baseline():
     assert CONFIGS[0] == dict(o=5, v=20, NL=60, NP=50, NX=100, seed=0)
     assert CONFIGS[4] == dict(o=250, v=2250, NL=7500, NP=5000, NX=10000, seed=4)
+
+
+def test_device_generator_matches_numpy_generator():
+    """thc_synth.device (torch ops; used on the GPU for configs 3-4) draws the same tensors as generators.py."""
+    import torch
+    from thc_synth import generators as g
+    from thc_synth import device as dv
+    idx = np.array([0, 1, 5, 123456789, 2 ** 40 + 7], dtype=np.uint64)
+    assert np.array_equal(g.uniform_block(3, 5, idx), dv.uniform_block(3, 5, torch.from_numpy(idx.astype(np.int64))).numpy())
+    x = g.make_inputs(3, 4, 6, 5, 7, seed=9)
+    d = dv.make_inputs_device(3, 4, 6, 5, 7, seed=9, device="cpu")
+    for k in ("eps", "Xo", "Xv", "Z", "B_oo", "B_ov", "B_vv", "Y", "V"):
+        assert np.abs(getattr(x, k) - d[k].numpy()).max() <= 1e-14, k
+    blk = dv.bvv_block(9, 3, 4, 6, 2, 5, "cpu").numpy()
+    assert np.abs(blk - x.B_vv[2:5]).max() <= 1e-14
