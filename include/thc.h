@@ -125,6 +125,27 @@ int thc_energy(thc_handle* h, const double* Xo, const double* Xv, const double* 
 int thc_energy_device(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
                       double* E_dev);
 
+/* ---- Sharded evaluation over several devices (one handle per device) -----
+ * The Cholesky index is cut into equal contiguous ranges (Alg.1/2/3/8 partial sums) and the amplitude-grid rows of the
+ * T2^2 terms (Alg.6/7) into equal contiguous row blocks:  thc_shard_range(NL, NP, rank, nranks, out) writes
+ * out = {L_begin, L_end, P_begin, P_end} (needs no device).
+ *   1. every rank calls thc_residual_shard with B_ov, B_oo, B_vv pointing at ITS OWN slice (vector L_begin first; the
+ *      slice may be empty, the pointers are then ignored) and a device buffer `packed` of thc_shard_doubles() doubles:
+ *      [sigma1 | sigma2 | C3 | sigma6 rows | sigma7 rows | C7 rows | xi_oo | xi_vv], rows of other ranks zero;
+ *   2. the caller sums `packed` element-wise over the ranks (one all-reduce; that is the only exchange step);
+ *   3. every rank calls thc_residual_finish with the summed buffer (it is modified): Alg.3 tail, Alg.9, the
+ *      C7 V C7^T part of Alg.7 and the final sum give R (and, if terms != NULL, each term; any entry may be NULL).
+ * thc_energy_shard writes the rank's partial energy (its Cholesky range) to E_dev; the caller sums over ranks. */
+int thc_shard_range(int64_t NL, int64_t NP, int rank, int nranks, int64_t out[4]);
+int64_t thc_shard_doubles(const thc_handle* h);
+int thc_residual_shard(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
+                       const double* B_oo, const double* B_vv, const double* Y, const double* V, const double* eps,
+                       int rank, int nranks, double* packed);
+int thc_residual_finish(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* Y,
+                        const double* V, const double* eps, double* packed, double* R, double* const terms[6]);
+int thc_energy_shard(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov, int rank,
+                     int nranks, double* E_dev);
+
 /* End-to-end entry with HOST buffers: copies every input host->device on the handle's stream, evaluates
  * R (and E if E_host != NULL), copies R device->host into R_host[NP][NP], synchronises.  The staging
  * buffers are part of the workspace (thc_workspace_bytes_host includes them).                       */

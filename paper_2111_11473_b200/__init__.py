@@ -22,7 +22,8 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
 SYMBOLS = ("thc_setup", "thc_destroy", "thc_workspace_bytes", "thc_workspace_bytes_host", "thc_set_workspace",
            "thc_set_stream", "thc_get_blocks", "thc_residual", "thc_residual_terms", "thc_energy",
            "thc_energy_device", "thc_residual_host", "thc_profile_begin", "thc_profile_end", "thc_kernel_launches", "thc_algorithmic_flops", "thc_dgemm",
-           "thc_triple_product", "thc_strerror", "thc_last_cuda_error")
+           "thc_triple_product", "thc_strerror", "thc_last_cuda_error", "thc_shard_range", "thc_shard_doubles",
+           "thc_residual_shard", "thc_residual_finish", "thc_energy_shard")
 
 TERM_NAMES = ("s1", "s2", "s3", "s6", "s7", "s9")
 TERM_BITS = dict(s1=1, s2=2, s3=4, s6=8, s7=16, s9=32)
@@ -106,6 +107,12 @@ def lib() -> ctypes.CDLL:
     L.thc_algorithmic_flops.restype = D
     L.thc_dgemm.argtypes = [VP, ctypes.c_int, ctypes.c_int, I64, I64, I64, D, P, I64, P, I64, D, P, I64]
     L.thc_triple_product.argtypes = [VP, I64, I64, I64, P, P, P, P, P, ctypes.c_int]
+    L.thc_shard_range.argtypes = [I64, I64, ctypes.c_int, ctypes.c_int, ctypes.POINTER(I64 * 4)]
+    L.thc_shard_doubles.argtypes = [VP]
+    L.thc_shard_doubles.restype = I64
+    L.thc_residual_shard.argtypes = [VP] + [P] * 9 + [ctypes.c_int, ctypes.c_int, P]
+    L.thc_residual_finish.argtypes = [VP] + [P] * 6 + [P, P, ctypes.POINTER(P * 6)]
+    L.thc_energy_shard.argtypes = [VP, P, P, P, P, ctypes.c_int, ctypes.c_int, P]
     L.thc_strerror.argtypes = [ctypes.c_int]
     L.thc_strerror.restype = ctypes.c_char_p
     L.thc_last_cuda_error.argtypes = [VP]
@@ -271,6 +278,59 @@ class Thc:
                                        _dev_ptr(E, "E", 1)), self._h)
         return E
 
+    # ---- sharded evaluation (one handle per device; the caller sums `packed` over the ranks) -------------------------
+    @property
+    def shard_doubles(self):
+        return int(lib().thc_shard_doubles(self._h))
+
+    def _slice_ptr(self, t, name, numel):
+        return ctypes.c_void_p(None) if numel == 0 else _dev_ptr(t, name, numel)
+
+    def thc_residual_shard(self, Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps, rank, nranks, out=None):
+        """This rank's packed partial sums (device tensor of shard_doubles); B_* are the rank's own L-slices."""
+        import torch
+        self._prepare(self.workspace_bytes)
+        o, v, NP, NX = self.o, self.v, self.NP, self.NX
+        L0, L1, _, _ = thc_shard_range(self.NL, NP, rank, nranks)
+        nl = L1 - L0
+        packed = out if out is not None else torch.empty(self.shard_doubles, dtype=torch.float64, device=self._device)
+        bvv = self._slice_ptr(B_vv, "B_vv", nl * v * v) if self.bvv_mode == "device" else self._bvv_ptr(B_vv, _dev_ptr)
+        _check(lib().thc_residual_shard(
+            self._h, _dev_ptr(Xo, "Xo", o * NP), _dev_ptr(Xv, "Xv", v * NP), _dev_ptr(Z, "Z", NP * NP),
+            self._slice_ptr(B_ov, "B_ov", nl * o * v), self._slice_ptr(B_oo, "B_oo", nl * o * o), bvv,
+            _dev_ptr(Y, "Y", (o + v) * NX), _dev_ptr(V, "V", NX * NX), _dev_ptr(eps, "eps", o + v), rank, nranks,
+            _dev_ptr(packed, "packed", self.shard_doubles)), self._h)
+        return packed
+
+    def thc_residual_finish(self, Xo, Xv, Z, Y, V, eps, packed, want_terms=False):
+        """R (and optionally every term) from the rank-summed packed buffer, which is modified."""
+        import torch
+        self._prepare(self.workspace_bytes)
+        o, v, NP, NX = self.o, self.v, self.NP, self.NX
+        kw = dict(dtype=torch.float64, device=self._device)
+        res = {"R": torch.empty(NP, NP, **kw)}
+        terms = None
+        if want_terms:
+            for k in TERM_NAMES:
+                res[k] = torch.empty(NP, NP, **kw)
+            terms = ctypes.byref((ctypes.c_void_p * 6)(*[res[k].data_ptr() for k in TERM_NAMES]))
+        _check(lib().thc_residual_finish(
+            self._h, _dev_ptr(Xo, "Xo", o * NP), _dev_ptr(Xv, "Xv", v * NP), _dev_ptr(Z, "Z", NP * NP),
+            _dev_ptr(Y, "Y", (o + v) * NX), _dev_ptr(V, "V", NX * NX), _dev_ptr(eps, "eps", o + v),
+            _dev_ptr(packed, "packed", self.shard_doubles), _dev_ptr(res["R"], "R"), terms), self._h)
+        return res if want_terms else res["R"]
+
+    def thc_energy_shard(self, Xo, Xv, Z, B_ov, rank, nranks, out=None):
+        import torch
+        self._prepare(self.workspace_bytes)
+        o, v, NP = self.o, self.v, self.NP
+        L0, L1, _, _ = thc_shard_range(self.NL, NP, rank, nranks)
+        E = out if out is not None else torch.empty(1, dtype=torch.float64, device=self._device)
+        _check(lib().thc_energy_shard(self._h, _dev_ptr(Xo, "Xo", o * NP), _dev_ptr(Xv, "Xv", v * NP),
+                                      _dev_ptr(Z, "Z", NP * NP), self._slice_ptr(B_ov, "B_ov", (L1 - L0) * o * v),
+                                      rank, nranks, _dev_ptr(E, "E", 1)), self._h)
+        return E
+
     def thc_profile_begin(self, class_mask=7):
         _check(lib().thc_profile_begin(self._h, int(class_mask)), self._h)
 
@@ -300,6 +360,13 @@ class Thc:
         _check(lib().thc_triple_product(self._h, nI, nPp, NPp, _dev_ptr(E, "E", nI * nPp * NPp),
                                         _dev_ptr(F, "F", nI * nPp * NPp), _dev_ptr(G, "G", nI * NPp * NPp), _dev_ptr(GT, "GT", nI * NPp * NPp),
                                         _dev_ptr(H, "H", nPp * NPp * NPp), int(accumulate)), self._h)
+
+
+def thc_shard_range(NL, NP, rank, nranks):
+    """(L_begin, L_end, P_begin, P_end) of one rank: its Cholesky range and its row block of the T2^2 terms."""
+    out = (ctypes.c_int64 * 4)()
+    _check(lib().thc_shard_range(NL, NP, rank, nranks, ctypes.byref(out)))
+    return tuple(int(x) for x in out)
 
 
 def thc_setup(o, v, NL, NP, NX, **options) -> Thc:

@@ -30,14 +30,36 @@ struct Outputs {
   double* xi_oo;
   double* xi_vv;
 };
+// Sharded evaluation: phase 1 computes one rank's partial
+// sums over its Cholesky range [Lb, Le) and its rows [Pb, Pe) of the T2^2 terms into `packed`; after the caller has
+// summed `packed` over the ranks, phase 2 finishes (Alg.3 tail, Alg.9, the C7 V C7^T part of Alg.7, the sum).
+// phase 0 is the ordinary single-device evaluation.  Packed layout: thc_shard_doubles().
+struct Shard {
+  int phase = 0;
+  i64 Lb = 0, Le = 0, Pb = 0, Pe = 0;
+  double* packed = nullptr;
+};
+struct PackedLayout {
+  i64 s1, s2, C3, s6, s7, C7, xi_oo, xi_vv, total;
+  PackedLayout(i64 o, i64 v, i64 NP, i64 NX) {
+    const i64 NP2 = NP * NP;
+    s1 = 0; s2 = NP2; C3 = 2 * NP2; s6 = 3 * NP2; s7 = 4 * NP2; C7 = 5 * NP2; xi_oo = C7 + NP * NX; xi_vv = xi_oo + o * o;
+    total = xi_vv + v * v;
+  }
+};
 
 inline i64 pad_to(i64 x, i64 m) { return (x + m - 1) / m * m; }
 
 // The whole residual evaluation.  Runs either for real or dry (workspace sizing); both take identical branches.
-void plan_residual(Ctx& c, const Inputs& in, const Outputs& out) {
+void plan_residual(Ctx& c, const Inputs& in, const Outputs& out, const Shard& sh = Shard()) {
   thc_handle* h = c.h;
   thc::Arena& ar = c.ar;
-  const i64 o = h->o, v = h->v, NL = h->NL, NP = h->NP, NX = h->NX;
+  const i64 o = h->o, v = h->v, NP = h->NP, NX = h->NX;
+  const bool local = sh.phase != 2;        // the L loop and the row blocks of Alg.6 / Alg.7
+  const bool post = sh.phase != 1;         // everything that needs the rank-summed intermediates
+  const i64 Lb = sh.phase ? sh.Lb : 0, Le = sh.phase ? sh.Le : h->NL, NL = Le - Lb;     // B_* point at vector Lb
+  const i64 Pb = sh.phase ? sh.Pb : 0, Pe = sh.phase ? sh.Pe : NP;
+  const PackedLayout pk(o, v, NP, NX);
   const i64 NP2 = NP * NP, ov = o * v;
   const int mask = h->term_mask ? h->term_mask : THC_TERM_ALL;
   const bool do_s1 = mask & THC_TERM_S1, do_s2 = mask & THC_TERM_S2, do_s3 = mask & THC_TERM_S3;
@@ -47,16 +69,21 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out) {
 
   // ---- persistent buffers -----------------------------------------------------------------------------------------
   double* term[6];
-  for (int k = 0; k < 6; k++) term[k] = out.terms[k] ? out.terms[k] : ar.alloc(NP2);
-  double *s1 = term[0], *s2 = term[1], *s3 = term[2], *s6 = term[3], *s7 = term[4], *s9 = term[5];
+  for (int k = 0; k < 6; k++) term[k] = out.terms[k] ? out.terms[k] : (sh.phase == 1 && (k == 2 || k == 5) ? nullptr : ar.alloc(NP2));
   double* xi_oo = out.xi_oo ? out.xi_oo : ar.alloc(o * o);
   double* xi_vv = out.xi_vv ? out.xi_vv : ar.alloc(v * v);
+  if (sh.phase) {                          // the summed quantities live in the packed buffer
+    term[0] = sh.packed + pk.s1; term[1] = sh.packed + pk.s2; term[3] = sh.packed + pk.s6; term[4] = sh.packed + pk.s7;
+    xi_oo = sh.packed + pk.xi_oo; xi_vv = sh.packed + pk.xi_vv;
+  }
+  double *s1 = term[0], *s2 = term[1], *s3 = term[2], *s6 = term[3], *s7 = term[4], *s9 = term[5];
   double* XoT = ar.alloc(NP * o);
   double* XvT = ar.alloc(NP * v);
   double* YoT = ar.alloc(NX * o);
   double* YvT = ar.alloc(NX * v);
-  double *omat = ar.alloc(NP2), *vmat = ar.alloc(NP2), *wmat = ar.alloc(NP2), *Kmat = ar.alloc(NP2), *C3 = ar.alloc(NP2);
-  double *Aa = ar.alloc(NL * NP), *Dm = ar.alloc(NL * NP);
+  double *omat = ar.alloc(NP2), *vmat = ar.alloc(NP2), *wmat = ar.alloc(NP2), *Kmat = ar.alloc(NP2);
+  double* C3 = sh.phase ? sh.packed + pk.C3 : ar.alloc(NP2);
+  double *Aa = ar.alloc(std::max<i64>(NL, 1) * NP), *Dm = ar.alloc(std::max<i64>(NL, 1) * NP);
 
   // ---- H0: transposed factors and grams (Alg.1 l.481-485) ------------------------------------------------------------
   c.transpose(in.Xo, XoT, o, NP);
@@ -67,14 +94,17 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out) {
   c.gemm(Gemm(XvT, v, 'K', XvT, v, 'K', vmat, NP, NP, NP, v));
   c.hadamard(omat, vmat, wmat, NP2);                                         // w = o .* v
   c.gemm(Gemm(wmat, NP, 'K', in.Z, NP, 'K', Kmat, NP, NP, NP, NP));           // K = w Z   (Z symmetric)
-  c.fill(C3, NP2, 0.0);
-  c.fill(s1, NP2, 0.0);
-  c.fill(xi_oo, o * o, 0.0);
-  c.fill(xi_vv, v * v, 0.0);
+  if (local) {
+    if (sh.phase == 1) c.fill(sh.packed, pk.total, 0.0);      // rows / terms this rank does not own stay zero
+    c.fill(C3, NP2, 0.0);
+    c.fill(s1, NP2, 0.0);
+    c.fill(xi_oo, o * o, 0.0);
+    c.fill(xi_vv, v * v, 0.0);
+  }
 
   // ---- L-block loop: Alg.1 + Alg.3 (H1-H4) and Alg.2 + Alg.8 (H5-H6) fused over the Cholesky index (l.238) ---------
-  const bool need_ladder = do_s1 || do_s3;
-  const bool need_ring = do_s2 || do_s9;
+  const bool need_ladder = local && (do_s1 || do_s3);
+  const bool need_ring = local && (do_s2 || do_s9);
   // B_vv source: resident (device pointer), or streamed one L-block at a time into a double buffer (l.191-195)
   const bool streamed = h->bvv_mode != THC_BVV_DEVICE && need_ladder;
   double* bvv_buf[2] = {nullptr, nullptr};
@@ -95,7 +125,7 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out) {
           if (L1 < NL) c.bvv_copy(bvv_buf[(blk + 1) & 1], in.B_vv, L1, std::min<i64>(h->bL, NL - L1), v, blk + 1);
           c.bvv_wait_loaded(blk);
         } else {
-          c.bvv_provide(reinterpret_cast<const thc_bvv_provider*>(in.B_vv), L0, nl, bvv_buf[blk & 1]);
+          c.bvv_provide(reinterpret_cast<const thc_bvv_provider*>(in.B_vv), Lb + L0, nl, bvv_buf[blk & 1]);
         }
       }
     }
@@ -148,7 +178,9 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out) {
   }
 
   // ---- H7: s2 = A A^T + Dm A^T + A Dm^T  (Alg.2 line 13 l.559; rows of Aa/Dm are Cholesky vectors) --------------------
-  if (do_s2) {
+  if (!local) {
+    // phase 2: s2 arrives summed over the ranks
+  } else if (do_s2 && NL > 0) {
     const i64 m0 = ar.mark();
     double* AD = ar.alloc(NL * NP);
     c.axpby(Aa, Dm, 1.0, 1.0, AD, NL * NP);
@@ -160,7 +192,9 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out) {
   }
 
   // ---- H8: Alg.3 tail and Alg.9 ------------------------------------------------------------------------------------
-  if (do_s3) {
+  if (!post) {
+    // phase 1: Alg.3 tail and Alg.9 need the rank-summed C3, xi_oo, xi_vv
+  } else if (do_s3) {
     // s3 = -(K C3^T + C3 K^T)                                                                        (Alg.3 line 12 l.601)
     const i64 m0 = ar.mark();
     double* P3 = ar.alloc(NP2);
@@ -170,7 +204,8 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out) {
   } else {
     c.fill(s3, NP2, 0.0);
   }
-  if (do_s9) {
+  if (!post) {
+  } else if (do_s9) {
     // F'_oo = diag(eps_o) + xi_oo, F'_vv = diag(eps_v) + xi_vv; o~ = Xo^T F'_oo^T.. (Alg.9 lines 5-10 l.823-839)
     const i64 m0 = ar.mark();
     double *FooT = ar.alloc(o * o), *Fvv = ar.alloc(v * v);
@@ -192,10 +227,12 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out) {
   // ---- H10: Alg.7, ring-type T2^2 terms with THC ERIs (Eqs.35-37 l.261-271; prefactor 1/2, R2) -----------
   if (do_s7) {
     const i64 m0 = ar.mark();
-    double *Rb = ar.alloc(NP * ov), *Sb = ar.alloc(NP * ov), *C7 = ar.alloc(NP * NX);
+    double* C7 = sh.phase ? sh.packed + pk.C7 : ar.alloc(NP * NX);
+    double *Rb = nullptr, *Sb = nullptr;
+    if (local) { Rb = ar.alloc(NP * ov); Sb = ar.alloc(NP * ov); }
     // pass 1 (Alg.7 lines 3-7): S^P = -(Xo .* v_P) Z (Xv .* o_P)^T ;  R^P = 2 (Xo .* K_P) Xv^T + S^P
     const i64 bA = std::min<i64>(NP, h->bP7 * 16);
-    for (i64 P0 = 0; P0 < NP; P0 += bA) {
+    for (i64 P0 = 0; local && P0 < NP; P0 += bA) {          // R^Q, S^Q are needed for every Q on every rank
       const i64 npb = std::min<i64>(bA, NP - P0), m1 = ar.mark();
       double *XoV = ar.alloc(npb * o * NP), *SZ = ar.alloc(npb * o * NP);
       c.rowscale(in.Xo, NP, vmat + P0 * NP, NP, nullptr, 1.0, XoV, npb, o, NP);
@@ -207,8 +244,8 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out) {
       ar.release(m1);
     }
     // pass 2 (lines 9-19): per P, E = Yo^T R^P Yv, F = E .* V, G^P = Yo F^T Yv^T; rows of s7 from G R^T and G~ S^T
-    for (i64 P0 = 0; P0 < NP; P0 += h->bP7) {
-      const i64 npb = std::min<i64>(h->bP7, NP - P0), m1 = ar.mark();
+    for (i64 P0 = Pb; local && P0 < Pe; P0 += h->bP7) {      // this rank's rows of sigma7
+      const i64 npb = std::min<i64>(h->bP7, Pe - P0), m1 = ar.mark();
       double *RYT = ar.alloc(npb * NX * o), *EF = ar.alloc(npb * NX * NX), *FYT = ar.alloc(npb * o * NX), *Gb = ar.alloc(npb * ov);
       for (int pass = 0; pass < 2; pass++) {
         const double* src = pass == 0 ? Rb : Sb;
@@ -221,17 +258,19 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out) {
       }
       ar.release(m1);
     }
-    // line 10 + first part of line 22: s7 += C7 V C7^T
-    double* CV = ar.alloc(NP * NX);
-    c.gemm(Gemm(C7, NX, 'K', in.V, NX, 'K', CV, NX, NP, NX, NX));
-    c.gemm(Gemm(CV, NX, 'K', C7, NX, 'K', s7, NP, NP, NP, NX).ab(1.0, 1.0));
+    // line 10 + first part of line 22: s7 += C7 V C7^T  (needs every row of C7: after the rank sum)
+    if (post) {
+      double* CV = ar.alloc(NP * NX);
+      c.gemm(Gemm(C7, NX, 'K', in.V, NX, 'K', CV, NX, NP, NX, NX));
+      c.gemm(Gemm(CV, NX, 'K', C7, NX, 'K', s7, NP, NP, NP, NX).ab(1.0, 1.0));
+    }
     ar.release(m0);
-  } else {
+  } else if (sh.phase == 0) {
     c.fill(s7, NP2, 0.0);
   }
 
   // ---- H9: Alg.6, ladder-type T2^2 terms with THC ERIs (Eq.34 l.254) -------------------------------------------------
-  if (do_s6) {
+  if (do_s6 && local) {
     const i64 m0 = ar.mark();
     const i64 NPp = pad_to(NP, thc::TP_RT);
     // line 1: A3[Q][i][a] = sum_S Z[Q,S] Xo[i,S] Xv[a,S]
@@ -244,8 +283,8 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out) {
       c.gemm(Gemm(ZX, NP, 'K', in.Xv, NP, 'K', A3 + P0 * ov, v, npb * o, v, NP));
       ar.release(m1);
     }
-    for (i64 P0 = 0; P0 < NP; P0 += h->bX) {
-      const i64 npb = std::min<i64>(h->bX, NP - P0), m1 = ar.mark();
+    for (i64 P0 = Pb; P0 < Pe; P0 += h->bX) {                // this rank's rows of sigma6
+      const i64 npb = std::min<i64>(h->bX, Pe - P0), m1 = ar.mark();
       const i64 bXp = pad_to(npb, thc::TP_PT);
       // lines 4-5: Cc[p][(q,i)] = sum_a Xv[a,P0+p] A3[q][i][a] ;  Dd[p][(q,a)] = sum_i Xo[i,P0+p] A3[q][i][a]
       double *Cc = ar.alloc(npb * NP * o), *Dd = ar.alloc(npb * NP * v), *H = ar.alloc(bXp * NPp * NPp);
@@ -281,7 +320,7 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out) {
       ar.release(m1);
     }
     ar.release(m0);
-  } else {
+  } else if (sh.phase == 0) {
     c.fill(s6, NP2, 0.0);
   }
 
@@ -291,10 +330,12 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out) {
 
 // Correlation energy, factorised (R7):  E = sum_L [ 2 a^L . Z a^L - sum_PQ Z_PQ E^L_PQ E^L_QP ],
 // a^L, E^L as in Alg.8 lines 5-6 (l.788-790).  Result in E_dev[0] (device).
-void plan_energy(Ctx& c, const double* Xo, const double* Xv, const double* Z, const double* B_ov, double* E_dev) {
+void plan_energy(Ctx& c, const double* Xo, const double* Xv, const double* Z, const double* B_ov, double* E_dev,
+                 i64 NL_local = -1) {
   thc_handle* h = c.h;
   thc::Arena& ar = c.ar;
-  const i64 o = h->o, v = h->v, NL = h->NL, NP = h->NP, NP2 = NP * NP, ov = o * v;
+  const i64 o = h->o, v = h->v, NL = NL_local >= 0 ? NL_local : h->NL, NP = h->NP, NP2 = NP * NP, ov = o * v;
+  if (NL == 0) { c.fill(E_dev, 1, 0.0); return; }          // a rank without Cholesky vectors contributes nothing
   const i64 nblk = (NL + h->bL - 1) / h->bL;
   double *XoT = ar.alloc(NP * o), *XvT = ar.alloc(NP * v), *Aa = ar.alloc(NL * NP), *ZA = ar.alloc(NL * NP);
   double* Eblk = ar.alloc(nblk);
@@ -387,23 +428,23 @@ struct DeviceGuard {
   ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
 };
 
-int run_residual(thc_handle* h, char* base, i64 bytes, const Inputs& in, const Outputs& out) {
+int run_residual(thc_handle* h, char* base, i64 bytes, const Inputs& in, const Outputs& out, const Shard& sh = Shard()) {
   Need need = dry_residual(h);
   Ctx c{h};
   int st = make_ctx(c, h, base, bytes, need);
   if (st != THC_OK) return st;
-  plan_residual(c, in, out);
+  plan_residual(c, in, out, sh);
   if (c.ar.overflow) return THC_ERR_NO_MEMORY;
   return c.status;
 }
 int run_energy(thc_handle* h, char* base, i64 bytes, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
-               double* E_host, double* E_dev) {
+               double* E_host, double* E_dev, i64 NL_local = -1) {
   Need need = dry_energy(h);
   Ctx c{h};
   int st = make_ctx(c, h, base, bytes, need);
   if (st != THC_OK) return st;
   double* e = c.ar.alloc(1);
-  plan_energy(c, Xo, Xv, Z, B_ov, E_dev ? E_dev : e);
+  plan_energy(c, Xo, Xv, Z, B_ov, E_dev ? E_dev : e, NL_local);
   if (c.ar.overflow) return THC_ERR_NO_MEMORY;
   if (c.status != THC_OK) return c.status;
   if (E_host) {
@@ -572,6 +613,79 @@ int thc_energy_device(thc_handle* h, const double* Xo, const double* Xv, const d
   int st = ensure_workspace(h, h->need_bytes);
   if (st != THC_OK) return st;
   return run_energy(h, static_cast<char*>(h->ws), h->ws_bytes, Xo, Xv, Z, B_ov, nullptr, E_dev);
+}
+
+// ---- sharded evaluation -----------------------------------------------------------------------------
+int thc_shard_range(int64_t NL, int64_t NP, int rank, int nranks, int64_t out[4]) {
+  if (!out || NL <= 0 || NP <= 0 || nranks <= 0 || rank < 0 || rank >= nranks) return THC_ERR_INVALID_ARG;
+  out[0] = NL * rank / nranks; out[1] = NL * (rank + 1) / nranks;          // equal contiguous Cholesky ranges (l.220)
+  out[2] = NP * rank / nranks; out[3] = NP * (rank + 1) / nranks;          // equal contiguous row blocks (l.257, l.273)
+  return THC_OK;
+}
+
+int64_t thc_shard_doubles(const thc_handle* h) {
+  return h ? PackedLayout(h->o, h->v, h->NP, h->NX).total : (int64_t)THC_ERR_INVALID_ARG;
+}
+
+int thc_residual_shard(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
+                       const double* B_oo, const double* B_vv, const double* Y, const double* V, const double* eps,
+                       int rank, int nranks, double* packed) {
+  if (!h || bad_ptr(Xo) || bad_ptr(Xv) || bad_ptr(Z) || bad_ptr(Y) || bad_ptr(V) || bad_ptr(eps) || bad_ptr(packed))
+    return THC_ERR_INVALID_ARG;
+  int64_t r[4];
+  int st = thc_shard_range(h->NL, h->NP, rank, nranks, r);
+  if (st != THC_OK) return st;
+  if (r[1] > r[0] && (bad_ptr(B_ov) || bad_ptr(B_oo) || bad_ptr(B_vv))) return THC_ERR_INVALID_ARG;
+  Inputs in{Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps};
+  Outputs out{};
+  Shard sh;
+  sh.phase = 1; sh.Lb = r[0]; sh.Le = r[1]; sh.Pb = r[2]; sh.Pe = r[3]; sh.packed = packed;
+  DeviceGuard g(h->device);
+  if (!g.ok) return THC_ERR_CUDA;
+  st = ensure_workspace(h, h->need_bytes);
+  if (st != THC_OK) return st;
+  return run_residual(h, static_cast<char*>(h->ws), h->ws_bytes, in, out, sh);
+}
+
+int thc_residual_finish(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* Y,
+                        const double* V, const double* eps, double* packed, double* R, double* const terms[6]) {
+  if (!h || bad_ptr(Xo) || bad_ptr(Xv) || bad_ptr(Z) || bad_ptr(Y) || bad_ptr(V) || bad_ptr(eps) || bad_ptr(packed) ||
+      bad_ptr(R))
+    return THC_ERR_INVALID_ARG;
+  Inputs in{Xo, Xv, Z, nullptr, nullptr, nullptr, Y, V, eps};
+  Outputs out{};
+  out.R = R;
+  if (terms) { out.terms[2] = terms[2]; out.terms[5] = terms[5]; }     // s3, s9; the other four live in `packed`
+  Shard sh;
+  sh.phase = 2; sh.packed = packed;
+  DeviceGuard g(h->device);
+  if (!g.ok) return THC_ERR_CUDA;
+  int st = ensure_workspace(h, h->need_bytes);
+  if (st != THC_OK) return st;
+  st = run_residual(h, static_cast<char*>(h->ws), h->ws_bytes, in, out, sh);
+  if (st != THC_OK || !terms) return st;
+  const PackedLayout pk(h->o, h->v, h->NP, h->NX);
+  const i64 off[6] = {pk.s1, pk.s2, -1, pk.s6, pk.s7, -1};
+  for (int k = 0; k < 6; k++)
+    if (off[k] >= 0 && terms[k]) {
+      cudaError_t e = cudaMemcpyAsync(terms[k], packed + off[k], (size_t)h->NP * h->NP * 8, cudaMemcpyDeviceToDevice, h->stream);
+      if (e != cudaSuccess) { h->last_cuda = (int)e; return THC_ERR_CUDA; }
+    }
+  return THC_OK;
+}
+
+int thc_energy_shard(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov, int rank,
+                     int nranks, double* E_dev) {
+  if (!h || bad_ptr(Xo) || bad_ptr(Xv) || bad_ptr(Z) || bad_ptr(E_dev)) return THC_ERR_INVALID_ARG;
+  int64_t r[4];
+  int st = thc_shard_range(h->NL, h->NP, rank, nranks, r);
+  if (st != THC_OK) return st;
+  if (r[1] > r[0] && bad_ptr(B_ov)) return THC_ERR_INVALID_ARG;
+  DeviceGuard g(h->device);
+  if (!g.ok) return THC_ERR_CUDA;
+  st = ensure_workspace(h, h->need_bytes);
+  if (st != THC_OK) return st;
+  return run_energy(h, static_cast<char*>(h->ws), h->ws_bytes, Xo, Xv, Z, B_ov, nullptr, E_dev, r[1] - r[0]);
 }
 
 int thc_profile_begin(thc_handle* h, int class_mask) {
