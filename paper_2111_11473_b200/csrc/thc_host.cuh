@@ -13,6 +13,7 @@
 #include "thc_gemm.cuh"
 #include "thc_kernels.cuh"
 #include "thc_triple.cuh"
+#include "thc_ring.cuh"
 
 struct thc_handle {
   int64_t o, v, NL, NP, NX;
@@ -310,6 +311,46 @@ struct Ctx {
     launched();
     prof_stop(2);
   }
+  // ---- Alg.7 lines 12-19 fused (o <= 64) ------------------------------------------------------------------------------
+  static bool ring_supported(i64 o) { return o <= 64; }
+  template <int KT>
+  void ring_launch(const RingParams& p, bool al16, dim3 grid) {
+    const int sm = ring_smem_bytes(KT);
+    if (al16) {
+      static bool done = false;
+      if (!done) { check(cudaFuncSetAttribute(ring_fused_kernel<KT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm)); done = true; }
+      ring_fused_kernel<KT, true><<<grid, RG_THREADS, sm, h->stream>>>(p);
+    } else {
+      static bool done = false;
+      if (!done) { check(cudaFuncSetAttribute(ring_fused_kernel<KT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm)); done = true; }
+      ring_fused_kernel<KT, false><<<grid, RG_THREADS, sm, h->stream>>>(p);
+    }
+  }
+  // FYT[b][j][I] = sum_J (sum_i YoT[I][i] RYT[b][J][i]) V[I][J] Yo[j][J]
+  void ring_fused(const double* YoT, const double* RYT, const double* V, const double* Yo, double* FYT, i64 NX, i64 o, i64 npb) {
+    if (dry || !ok()) return;
+    RingParams p;
+    p.YoT = YoT; p.RYT = RYT; p.V = V; p.Yo = Yo; p.FYT = FYT; p.NX = (int)NX; p.o = (int)o; p.npb = (int)npb;
+    const bool al16 = (o % 2 == 0) && (NX % 2 == 0) &&
+                      ((reinterpret_cast<uintptr_t>(RYT) | reinterpret_cast<uintptr_t>(V) | reinterpret_cast<uintptr_t>(Yo)) & 15) == 0;
+    dim3 grid((unsigned)((NX + RG_BM - 1) / RG_BM), (unsigned)npb);
+    char desc[96];
+    if (h->prof_mask & 1) snprintf(desc, sizeof desc, "ring_fused NX=%d o=%d batch=%d", (int)NX, (int)o, (int)npb);
+    prof_start(0, desc, 4.0 * o * (double)NX * NX * npb);
+    switch ((o + 7) / 8) {
+      case 1: ring_launch<1>(p, al16, grid); break;
+      case 2: ring_launch<2>(p, al16, grid); break;
+      case 3: ring_launch<3>(p, al16, grid); break;
+      case 4: ring_launch<4>(p, al16, grid); break;
+      case 5: ring_launch<5>(p, al16, grid); break;
+      case 6: ring_launch<6>(p, al16, grid); break;
+      case 7: ring_launch<7>(p, al16, grid); break;
+      default: ring_launch<8>(p, al16, grid); break;
+    }
+    launched();
+    prof_stop(0);
+  }
+
   // ---- B_vv streaming (THC_BVV_HOST / THC_BVV_PROVIDER) ------------------------------------------------------------
   void bvv_begin() {
     if (!ok() || h->bvv_mode != THC_BVV_HOST) return;

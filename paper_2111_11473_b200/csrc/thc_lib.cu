@@ -246,13 +246,18 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out, const Shard& sh
     // pass 2 (lines 9-19): per P, E = Yo^T R^P Yv, F = E .* V, G^P = Yo F^T Yv^T; rows of s7 from G R^T and G~ S^T
     for (i64 P0 = Pb; local && P0 < Pe; P0 += h->bP7) {      // this rank's rows of sigma7
       const i64 npb = std::min<i64>(h->bP7, Pe - P0), m1 = ar.mark();
-      double *RYT = ar.alloc(npb * NX * o), *EF = ar.alloc(npb * NX * NX), *FYT = ar.alloc(npb * o * NX), *Gb = ar.alloc(npb * ov);
+      const bool fused = Ctx::ring_supported(o);       // E and F = E .* V stay in registers (thc_ring.cuh)
+      double *RYT = ar.alloc(npb * NX * o), *EF = fused ? nullptr : ar.alloc(npb * NX * NX), *FYT = ar.alloc(npb * o * NX), *Gb = ar.alloc(npb * ov);
       for (int pass = 0; pass < 2; pass++) {
         const double* src = pass == 0 ? Rb : Sb;
         c.gemm(Gemm(YvT, v, 'K', src + P0 * ov, v, 'K', RYT, o, NX, o, v).batch(npb, 0, ov, NX * o));
         if (pass == 0) c.rowdot(YoT, o, RYT, NX * o, o, C7 + P0 * NX, NX, npb, NX, o);     // line 9
-        c.gemm(Gemm(YoT, o, 'K', RYT, o, 'K', EF, NX, NX, NX, o).batch(npb, 0, NX * o, NX * NX).aux(in.V, NX, 0));
-        c.gemm(Gemm(Yo, NX, 'K', EF, NX, 'K', FYT, NX, o, NX, NX).batch(npb, 0, NX * NX, o * NX));
+        if (fused) {
+          c.ring_fused(YoT, RYT, in.V, Yo, FYT, NX, o, npb);
+        } else {
+          c.gemm(Gemm(YoT, o, 'K', RYT, o, 'K', EF, NX, NX, NX, o).batch(npb, 0, NX * o, NX * NX).aux(in.V, NX, 0));
+          c.gemm(Gemm(Yo, NX, 'K', EF, NX, 'K', FYT, NX, o, NX, NX).batch(npb, 0, NX * NX, o * NX));
+        }
         c.gemm(Gemm(FYT, NX, 'K', Yv, NX, 'K', Gb, v, npb * o, v, NX));
         c.gemm(Gemm(Gb, ov, 'K', src, ov, 'K', s7 + P0 * NP, NP, npb, NP, ov).ab(pass == 0 ? -0.5 : 0.5, pass == 0 ? 0.0 : 1.0));
       }
@@ -494,8 +499,9 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
   h->bvv_mode = opt ? opt->bvv_mode : THC_BVV_DEVICE; h->copy_stream = nullptr; h->copy_ready = false;
 
   // block sizes: defaults, then shrink until the plan fits the cap
-  h->bL = std::min<int64_t>(NL, (opt && opt->bL) ? opt->bL : 32);
-  const int64_t p7_auto = std::max<int64_t>(1, ((int64_t)2 << 30) / (NX * NX * 8));
+  h->bL = std::min<int64_t>(NL, (opt && opt->bL) ? opt->bL : 512);    // long L-blocks: few, large GEMMs (shrunk below if HBM is short)
+  const int64_t p7_auto = o <= 64 ? std::max<int64_t>(1, ((int64_t)2 << 30) / (NX * (o + v) * 8 + 1))
+                                  : std::max<int64_t>(1, ((int64_t)2 << 30) / (NX * NX * 8));
   h->bP7 = std::min<int64_t>(NP, (opt && opt->bP7) ? opt->bP7 : p7_auto);
   h->bX = std::min<int64_t>(pad_to(NP, 16), (opt && opt->bX) ? pad_to(opt->bX, 16) : pad_to(NP, 16));
   h->bI = std::min<int64_t>(NX, (opt && opt->bI) ? opt->bI : 512);   // long I loops amortise the H read-modify-write
@@ -507,6 +513,16 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
     cap = (int64_t)(0.75 * (double)fr);
   }
   const bool fix_bX = opt && opt->bX, fix_bI = opt && opt->bI, fix_bP7 = opt && opt->bP7, fix_bL = opt && opt->bL;
+  {
+    // stage A: the L-block loop and the T2^2 phases reuse the same arena, so first find the largest bL whose own phase
+    // fits (the other block sizes at their minimum), then size the rest with bL fixed
+    const int64_t sX = h->bX, sP = h->bP7, sI = h->bI;
+    if (!fix_bX) h->bX = 16;
+    if (!fix_bP7) h->bP7 = 1;
+    if (!fix_bI) h->bI = std::min<int64_t>(NX, 16);
+    while (!fix_bL && h->bL > 1 && need_device(h) > cap) h->bL = h->bL / 2;
+    h->bX = sX; h->bP7 = sP; h->bI = sI;
+  }
   for (;;) {
     h->need_bytes = need_device(h);
     if (h->need_bytes <= cap) break;
