@@ -258,6 +258,7 @@ def run_ours(args):
     h.thc_profile_begin(7)
     step()
     prof_w = h.thc_profile_end()
+    work_w = h.thc_profile_work()        # executed flop (gemm, triple) / algorithmic HBM bytes (ew) of that step
     dominant = max(prof_w, key=lambda k: prof_w[k][0])
     dom_bit = {"gemm": 1, "triple": 2, "ew": 4}[dominant]
 
@@ -353,6 +354,19 @@ def run_ours(args):
     roof["ms_per_step"] = per_eval_ms
     roof["share_of_step"] = per_eval_ms / (1e3 * total_s / K)
     roof["class_ms_warmup_step"] = {k: round(prof_w[k][0], 4) for k in prof_w}
+    # every kernel class of one profiled warm-up step against its own roof (EXECUTED work, recomputation included)
+    dmma_probe = SMS * DFMA_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
+    per_class = {}
+    for k, (unit, peak, bound) in {"gemm": ("TFLOP/s", pk["bf16"] * NOMINAL_FP64_TENSOR_OVER_BF16, "tensor"),
+                                   "triple": ("TFLOP/s", dmma_probe, "alu"),
+                                   "ew": ("GB/s", pk["hbm"], "hbm")}.items():
+        ms_k = prof_w[k][0]
+        if ms_k <= 0:
+            continue
+        ach = work_w[k] / (ms_k * 1e-3) / (1e12 if unit == "TFLOP/s" else 1e9)
+        per_class[k] = {"bound": bound, "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak,
+                        "ms": round(ms_k, 4), "launches": prof_w[k][1]}
+    per_class["gemm"]["frac_of_dmma_issue_rate"] = per_class["gemm"]["achieved"] / dmma_probe if "gemm" in per_class else None
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": 1e3 * total_s / K, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
@@ -366,7 +380,7 @@ def run_ours(args):
             "wall_s_timed_region": wall, "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": input_bytes, "d2h_bytes_per_step": NP * NP * 8 + 8,
                     "steps": Ke},
-            "gpu_launches": launches, "roofline": roof}
+            "gpu_launches": launches, "roofline": roof, "rooflines_by_class": per_class}
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = time_oracle(args.config, reps=3)
     print(json.dumps(line), flush=True)

@@ -165,6 +165,10 @@ double thc_algorithmic_flops(const thc_handle* h);
  * launches per class, and switches the timing off again.  Not for use while the stream is being captured. */
 int thc_profile_begin(thc_handle* h, int class_mask);
 int thc_profile_end(thc_handle* h, double ms[3], int64_t counts[3]);
+/* Work of the launches timed by the last thc_profile_end, per class: EXECUTED flop for classes 0 and 1 (every GEMM
+ * launched, recomputation included; 5 flop per (P,Q,R,I) of line 11 over the padded extents), algorithmic HBM bytes
+ * (each operand element read once, each result written once) for class 2. */
+int thc_profile_work(const thc_handle* h, double work[3]);
 
 /* Bare FP64 DMMA GEMM of the library (the kernel every GEMM chain uses), exposed for tests and roofline
  * measurement:  C[M][N] = alpha * sum_k A(m,k) B(n,k) + beta * C,  A(m,k) = A[m*lda+k] if a_kmajor else

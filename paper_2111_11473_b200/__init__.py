@@ -21,7 +21,7 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
 # every symbol include/thc.h declares
 SYMBOLS = ("thc_setup", "thc_destroy", "thc_workspace_bytes", "thc_workspace_bytes_host", "thc_set_workspace",
            "thc_set_stream", "thc_get_blocks", "thc_residual", "thc_residual_terms", "thc_energy",
-           "thc_energy_device", "thc_residual_host", "thc_profile_begin", "thc_profile_end", "thc_kernel_launches", "thc_algorithmic_flops", "thc_dgemm",
+           "thc_energy_device", "thc_residual_host", "thc_profile_begin", "thc_profile_end", "thc_profile_work", "thc_kernel_launches", "thc_algorithmic_flops", "thc_dgemm",
            "thc_triple_product", "thc_strerror", "thc_last_cuda_error", "thc_shard_range", "thc_shard_doubles",
            "thc_residual_shard", "thc_residual_finish", "thc_energy_shard")
 
@@ -100,6 +100,7 @@ def lib() -> ctypes.CDLL:
     L.thc_energy_device.argtypes = [VP, P, P, P, P, P]
     L.thc_profile_begin.argtypes = [VP, ctypes.c_int]
     L.thc_profile_end.argtypes = [VP, ctypes.POINTER(D * 3), ctypes.POINTER(I64 * 3)]
+    L.thc_profile_work.argtypes = [VP, ctypes.POINTER(D * 3)]
     L.thc_residual_host.argtypes = [VP] + [P] * 10 + [ctypes.POINTER(D)]
     L.thc_kernel_launches.argtypes = [VP]
     L.thc_kernel_launches.restype = I64
@@ -219,7 +220,10 @@ class Thc:
 
         def _fill(ctx, L0, nl, dst, stream):
             try:
-                with torch.cuda.stream(torch.cuda.ExternalStream(stream or 0, device=self._device)):
+                # ExternalStream(0) would hand out a NEW pool stream, not the legacy default stream the library is on
+                lib_stream = (torch.cuda.ExternalStream(stream, device=self._device) if stream
+                              else torch.cuda.default_stream(self._device))
+                with torch.cuda.stream(lib_stream):
                     B_vv(int(L0), int(nl), torch.as_tensor(_DevView(dst, (nl, v, v)), device=self._device))
                 return 0
             except Exception as exc:            # never let an exception cross the C ABI
@@ -339,6 +343,12 @@ class Thc:
         ms, cnt = (ctypes.c_double * 3)(), (ctypes.c_int64 * 3)()
         _check(lib().thc_profile_end(self._h, ctypes.byref(ms), ctypes.byref(cnt)), self._h)
         return {k: (ms[i], cnt[i]) for i, k in enumerate(("gemm", "triple", "ew"))}
+
+    def thc_profile_work(self):
+        """{class: executed flop (gemm, triple) or algorithmic HBM bytes (ew)} of the last thc_profile_end."""
+        w = (ctypes.c_double * 3)()
+        _check(lib().thc_profile_work(self._h, ctypes.byref(w)), self._h)
+        return {k: w[i] for i, k in enumerate(("gemm", "triple", "ew"))}
 
     def thc_residual_host(self, Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps, R_host, want_energy=True):
         """End-to-end entry: HOST tensors in, R written into the host tensor R_host, returns E (or None)."""

@@ -43,7 +43,8 @@ struct thc_handle {
   std::vector<cudaEvent_t> prof_events;     // pool; pairs (start, stop)
   std::vector<int> prof_class;              // class of pair k
   std::vector<std::string> prof_desc;       // what pair k timed (printed by thc_profile_end when THC_TRACE is set)
-  std::vector<double> prof_flops;
+  std::vector<double> prof_flops;          // flop (classes 0, 1) or algorithmic HBM bytes (class 2) of pair k
+  double prof_work[3];                      // summed over the launches of the last thc_profile_end
   size_t prof_used;                         // pairs in use
 };
 
@@ -85,7 +86,11 @@ struct Gemm {
 };
 
 // tile configurations of dgemm_kernel
-#define THC_BIG 128, 128, 16, 2, 4, 4
+#ifndef THC_BIG_BK
+#define THC_BIG_BK 16
+#define THC_BIG_ST 4
+#endif
+#define THC_BIG 128, 128, THC_BIG_BK, 2, 4, THC_BIG_ST
 #define THC_SMALL 64, 64, 16, 2, 2, 4
 constexpr int BIG_THREADS = 256, SMALL_THREADS = 128;
 constexpr int gemm_smem_bytes(int BM, int BN, int BK, int ST, bool akm, bool bkm) {
@@ -96,7 +101,7 @@ template <bool AKM, bool BKM, bool AL16>
 static cudaError_t launch_gemm_variant(bool big, dim3 grid, cudaStream_t st, const GemmParams& p) {
   if (big) {
     auto k = dgemm_kernel<THC_BIG, AKM, BKM, AL16>;
-    int sm = gemm_smem_bytes(128, 128, 16, 4, AKM, BKM);
+    int sm = gemm_smem_bytes(128, 128, THC_BIG_BK, THC_BIG_ST, AKM, BKM);
     static bool done = false;
     if (!done) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, sm); done = true; }
     k<<<grid, BIG_THREADS, sm, st>>>(p);
@@ -227,10 +232,11 @@ struct Ctx {
   }
 
   // ---- element-wise / reduction launches -------------------------------------------------------------------------
-#define THC_EW(kernel, n, ...)                                          \
+// `bytes` = algorithmic HBM bytes of the launch (every operand element read once, every result written once)
+#define THC_EW(kernel, n, bytes, ...)                                   \
   do {                                                                  \
     if (dry || !ok()) return;                                           \
-    prof_start(2, #kernel, (double)(n));                                                    \
+    prof_start(2, #kernel, (double)(bytes));                            \
     kernel<<<ew_blocks(n), 256, 0, h->stream>>>(__VA_ARGS__);           \
     launched();                                                         \
     prof_stop(2);                                                       \
@@ -239,57 +245,57 @@ struct Ctx {
   void transpose(const double* in, double* out, i64 rows, i64 cols) {
     if (dry || !ok()) return;
     dim3 grid((unsigned)((cols + 31) / 32), (unsigned)((rows + 31) / 32)), blk(32, 8);
-    prof_start(2);
+    prof_start(2, "transpose_kernel", 16.0 * rows * cols);
     transpose_kernel<<<grid, blk, 0, h->stream>>>(in, out, (int)rows, (int)cols);
     launched();
     prof_stop(2);
   }
-  void fill(double* x, i64 n, double val) { THC_EW(fill_kernel, n, x, n, val); }
-  void hadamard(const double* a, const double* b, double* out, i64 n) { THC_EW(hadamard_kernel, n, a, b, out, n); }
+  void fill(double* x, i64 n, double val) { THC_EW(fill_kernel, n, 8.0 * n, x, n, val); }
+  void hadamard(const double* a, const double* b, double* out, i64 n) { THC_EW(hadamard_kernel, n, 24.0 * n, a, b, out, n); }
   void axpby(const double* a, const double* b, double ca, double cb, double* out, i64 n) {
-    THC_EW(axpby_kernel, n, a, b, ca, cb, out, n);
+    THC_EW(axpby_kernel, n, 24.0 * n, a, b, ca, cb, out, n);
   }
   void had2_diff(const double* a, const double* b, const double* c, const double* d, double* out, i64 n) {
-    THC_EW(had2_diff_kernel, n, a, b, c, d, out, n);
+    THC_EW(had2_diff_kernel, n, 40.0 * n, a, b, c, d, out, n);
   }
   void combine(double* Mo, const double* Mv, const double* omat, const double* vmat, double* C3, i64 np2, i64 nl) {
-    THC_EW(combine_kernel, np2, Mo, Mv, omat, vmat, C3, np2, (int)nl);
+    THC_EW(combine_kernel, np2, 8.0 * np2 * (3.0 * nl + 4.0), Mo, Mv, omat, vmat, C3, np2, (int)nl);
   }
   void rowdot(const double* X, i64 ldx, const double* T, i64 sTb, i64 ldT, double* out, i64 ldo, i64 nb, i64 nr, i64 n) {
-    THC_EW(rowdot_kernel, nb * nr, X, ldx, T, sTb, ldT, out, ldo, (int)nb, (int)nr, (int)n);
+    THC_EW(rowdot_kernel, nb * nr, 8.0 * ((double)nb * nr * n + (double)nr * n + (double)nb * nr), X, ldx, T, sTb, ldT, out, ldo, (int)nb, (int)nr, (int)n);
   }
   void coldot(const double* X, i64 ldx, const double* T, i64 sTb, i64 ldT, double* out, i64 ldo, i64 nb, i64 nc, i64 n) {
-    THC_EW(coldot_kernel, nb * nc, X, ldx, T, sTb, ldT, out, ldo, (int)nb, (int)nc, (int)n);
+    THC_EW(coldot_kernel, nb * nc, 8.0 * ((double)nb * nc * n + (double)nc * n + (double)nb * nc), X, ldx, T, sTb, ldT, out, ldo, (int)nb, (int)nc, (int)n);
   }
   void rowscale(const double* X, i64 ldx, const double* Mrow, i64 ldm, const double* add, double alpha, double* out,
                 i64 nb, i64 n, i64 nc) {
-    THC_EW(rowscale_kernel, nb * n * nc, X, ldx, Mrow, ldm, add, alpha, out, (int)nb, (int)n, (int)nc);
+    THC_EW(rowscale_kernel, nb * n * nc, 8.0 * ((double)nb * n * nc * (add ? 2.0 : 1.0) + (double)n * nc + (double)nb * nc), X, ldx, Mrow, ldm, add, alpha, out, (int)nb, (int)n, (int)nc);
   }
   void rowscale_inplace(double* T, const double* Mrow, i64 ldm, double alpha, i64 nb, i64 n, i64 nc) {
-    THC_EW(rowscale_inplace_kernel, nb * n * nc, T, Mrow, ldm, alpha, (int)nb, (int)n, (int)nc);
+    THC_EW(rowscale_inplace_kernel, nb * n * nc, 8.0 * (2.0 * nb * n * nc + (double)nb * nc), T, Mrow, ldm, alpha, (int)nb, (int)n, (int)nc);
   }
   void qm(double* G1, const double* Xo, const double* ZA, i64 o, i64 nl, i64 NP) {
-    THC_EW(qm_kernel, o * nl * NP, G1, Xo, ZA, (int)o, (int)nl, (int)NP);
+    THC_EW(qm_kernel, o * nl * NP, 8.0 * (2.0 * o * nl * NP + (double)o * NP + (double)nl * NP), G1, Xo, ZA, (int)o, (int)nl, (int)NP);
   }
   void symmetrize(const double* P, double* out, i64 n, double scale) {
     if (dry || !ok()) return;
     dim3 grid((unsigned)((n + 31) / 32), (unsigned)((n + 31) / 32)), blk(32, 8);
-    prof_start(2);
+    prof_start(2, "symmetrize_kernel", 16.0 * n * n);
     symmetrize_kernel<<<grid, blk, 0, h->stream>>>(P, out, (int)n, scale);
     launched();
     prof_stop(2);
   }
   void fock(const double* eps, const double* xi_oo, const double* xi_vv, double* FooT, double* Fvv, i64 o, i64 v) {
-    THC_EW(fock_kernel, o * o + v * v, eps, xi_oo, xi_vv, FooT, Fvv, (int)o, (int)v);
+    THC_EW(fock_kernel, o * o + v * v, 16.0 * (o * o + v * v), eps, xi_oo, xi_vv, FooT, Fvv, (int)o, (int)v);
   }
   void sum6(const double* const t[6], double* out, i64 n) {
-    THC_EW(sum6_kernel, n, t[0], t[1], t[2], t[3], t[4], t[5], out, n);
+    THC_EW(sum6_kernel, n, 56.0 * n, t[0], t[1], t[2], t[3], t[4], t[5], out, n);
   }
   // partial sums for the energy; `partial` must hold dot_blocks() / zee_blocks() doubles
   int dot_blocks(i64 n) const { return ew_blocks(n, 1024); }
   void dot_partial(const double* a, const double* b, i64 n, double* partial) {
     if (dry || !ok()) return;
-    prof_start(2);
+    prof_start(2, "dot_partial_kernel", 16.0 * n);
     dot_partial_kernel<<<dot_blocks(n), 256, 0, h->stream>>>(a, b, n, partial);
     launched();
     prof_stop(2);
@@ -299,14 +305,14 @@ struct Ctx {
     if (dry || !ok()) return;
     unsigned t = (unsigned)((NP + 31) / 32);
     dim3 grid(t, t, (unsigned)nl), blk(32, 8);
-    prof_start(2);
+    prof_start(2, "zee_partial_kernel", 8.0 * NP * NP * (nl + 1.0));
     zee_partial_kernel<<<grid, blk, 0, h->stream>>>(Z, E, (int)NP, partial);
     launched();
     prof_stop(2);
   }
   void final_sum(const double* pa, i64 na, double ca, const double* pb, i64 nb, double cb, double* out, int accumulate) {
     if (dry || !ok()) return;
-    prof_start(2);
+    prof_start(2, "final_sum_kernel", 8.0 * (na + nb));
     final_sum_kernel<<<1, 1024, 0, h->stream>>>(pa, na, ca, pb, nb, cb, out, accumulate);
     launched();
     prof_stop(2);

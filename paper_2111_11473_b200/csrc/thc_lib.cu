@@ -496,6 +496,7 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
   h->stream = nullptr; h->ws = nullptr; h->ws_bytes = 0; h->ws_owned = false;
   h->launches = 0; h->last_cuda = 0; h->smem_configured = false;
   h->prof_mask = 0; h->prof_used = 0; h->encode_tiled = nullptr;
+  h->prof_work[0] = h->prof_work[1] = h->prof_work[2] = 0.0;
   h->bvv_mode = opt ? opt->bvv_mode : THC_BVV_DEVICE; h->copy_stream = nullptr; h->copy_ready = false;
 
   // block sizes: defaults, then shrink until the plan fits the cap
@@ -715,7 +716,7 @@ int thc_profile_end(thc_handle* h, double ms[3], int64_t counts[3]) {
   if (!h || !ms || !counts) return THC_ERR_INVALID_ARG;
   DeviceGuard g(h->device);
   if (!g.ok) return THC_ERR_CUDA;
-  for (int k = 0; k < 3; k++) { ms[k] = 0.0; counts[k] = 0; }
+  for (int k = 0; k < 3; k++) { ms[k] = 0.0; counts[k] = 0; h->prof_work[k] = 0.0; }
   cudaError_t e = cudaStreamSynchronize(h->stream);
   if (e != cudaSuccess) { h->last_cuda = (int)e; return THC_ERR_CUDA; }
   const bool trace = getenv("THC_TRACE") != nullptr;     // developer aid: one stderr line per timed launch
@@ -728,9 +729,16 @@ int thc_profile_end(thc_handle* h, double ms[3], int64_t counts[3]) {
               h->prof_desc[k].c_str());
     ms[h->prof_class[k]] += (double)t;
     counts[h->prof_class[k]]++;
+    h->prof_work[h->prof_class[k]] += h->prof_flops[k];
   }
   h->prof_mask = 0;
   h->prof_used = 0;
+  return THC_OK;
+}
+
+int thc_profile_work(const thc_handle* h, double work[3]) {
+  if (!h || !work) return THC_ERR_INVALID_ARG;
+  for (int k = 0; k < 3; k++) work[k] = h->prof_work[k];
   return THC_OK;
 }
 

@@ -129,18 +129,43 @@ def test_streamed_bvv_matches_resident(mode):
     h0.close()
     h = thc.thc_setup(x.o, x.v, x.NL, x.NP, x.NX, bL=4, bvv_mode=mode)
     calls = []
+    lib_stream = torch.cuda.current_stream().cuda_stream
     if mode == "host":
         bvv = torch.from_numpy(np.ascontiguousarray(x.B_vv)).pin_memory()
     else:
         def bvv(L0, nl, dst):
             calls.append((L0, nl))
+            assert torch.cuda.current_stream().cuda_stream == lib_stream      # fills must be ordered with the GEMMs
             dst.copy_(d[5][L0:L0 + nl])
     args = list(d)
     args[5] = bvv
     for _ in range(2):                      # twice: the double buffer must be reusable across calls
         R = h.thc_residual(*args).cpu().numpy()
         assert np.array_equal(R, R0)
+        assert getattr(h, "_provider_error", None) is None, h._provider_error
     assert _relerr(R, ref["R"]) <= RTOL
     if mode == "provider":
         assert calls[:3] == [(0, 4), (4, 4), (8, 4)] and calls[5] == (20, 1)
+    h.close()
+
+
+def test_provider_fill_is_stream_ordered_at_scale():
+    """A fast provider (device-to-device copy) on a problem large enough that an unordered fill would overwrite the
+    double buffer before the previous block's GEMM has read it (regression: fills once ran on a torch pool stream)."""
+    import torch
+    import paper_2111_11473_b200 as thc
+    from thc_synth.device import make_inputs_device
+    o, v, NL, NP, NX = 16, 256, 96, 320, 64
+    d = make_inputs_device(o, v, NL, NP, NX, seed=12)
+    names = ("Xo", "Xv", "Z", "B_ov", "B_oo", "B_vv", "Y", "V", "eps")
+    mask = thc.TERM_BITS["s1"] | thc.TERM_BITS["s3"]
+    h0 = thc.thc_setup(o, v, NL, NP, NX, bL=8, term_mask=mask)
+    ref = h0.thc_residual(*[d[n] for n in names]).clone()
+    h0.close()
+    h = thc.thc_setup(o, v, NL, NP, NX, bL=8, term_mask=mask, bvv_mode="provider")
+    args = [d[n] for n in names]
+    args[5] = lambda L0, nl, dst: dst.copy_(d["B_vv"][L0:L0 + nl])
+    for _ in range(3):
+        R = h.thc_residual(*args)
+        assert torch.equal(R, ref)
     h.close()
