@@ -3,7 +3,8 @@
 //   C_b[m][n] = alpha * ( sum_{kb < kbatch} sum_{k < K} A_{b,kb}(m,k) * B_{b,kb}(n,k) ) (.* aux_b[m][n]) + beta * C_b[m][n]
 //
 // A(m,k) = A[m*lda + k] ("K-major") or A[k*lda + m] ("M-major"); likewise B(n,k).  `kbatch` is a second,
-// strided K loop (sum over Cholesky vectors of D^L C^L^T, Alg.1 line 15 l.524); `splits` cuts the
+// strided K loop (sum over Cholesky vectors of D^L C^L^T, Alg.1 line 15 l.524); `Ct` is an optional transposed copy
+// of the product (Alg.6 needs G_I in both orientations); `splits` cuts the
 // combined K range over grid.z and writes partial tiles that reduce_splits_kernel adds up in a fixed order.
 //
 // Tensor-core path: on sm_100a every FP64 mma.sync shape is issued as DMMA.8x8x4 (checked with cuobjdump),
@@ -27,6 +28,7 @@ struct GemmParams {
   int kbatch; long long sAk, sBk;
   int splits; long long sCs;      // split-K: partial tile stride (C then points at the partial buffer)
   double alpha, beta;
+  double* Ct; long long ldct, sCtb;   // optional second output: Ct_b[n][m] = alpha * (A B^T)[m][n] (no aux, no beta)
 };
 
 __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
@@ -227,6 +229,11 @@ __global__ void __launch_bounds__(WM* WN * 32) dgemm_kernel(const GemmParams p) 
           v0 *= auxb[(long long)m * p.ldaux + n];
           if (two) v1 *= auxb[(long long)m * p.ldaux + n + 1];
         }
+      }
+      if (p.Ct != nullptr && !partial) {          // transposed copy, before aux / beta are applied to the main output
+        double* ct = p.Ct + (long long)b * p.sCtb + (long long)n * p.ldct + m;
+        ct[0] = acc[i][j][0] * p.alpha;
+        if (two) ct[p.ldct] = acc[i][j][1] * p.alpha;
       }
       double* c = Cb + (long long)m * p.ldc + n;
       if (!partial && p.beta != 0.0) {

@@ -76,6 +76,7 @@ struct Gemm {
   int nkb = 1; i64 sAk = 0, sBk = 0;
   double alpha_ = 1.0, beta_ = 0.0;
   const double* aux_ = nullptr; i64 ldaux = 0, sAuxb = 0;
+  double* ct_ = nullptr; i64 ldct = 0, sCtb = 0;
   // A(m,k): am == 'K' -> A[m*lda + k], 'M' -> A[k*lda + m].  B(n,k): bm == 'K' -> B[n*ldb + k], 'N' -> B[k*ldb + n].
   Gemm(const double* A_, i64 lda_, char am, const double* B_, i64 ldb_, char bm, double* C_, i64 ldc_, i64 M_, i64 N_, i64 K_)
       : M((int)M_), N((int)N_), K((int)K_), A(A_), lda(lda_), akm(am == 'K'), B(B_), ldb(ldb_), bkm(bm == 'K'), C(C_), ldc(ldc_) {}
@@ -83,6 +84,7 @@ struct Gemm {
   Gemm& kbatch(i64 n, i64 sa, i64 sb) { nkb = (int)n; sAk = sa; sBk = sb; return *this; }
   Gemm& ab(double a, double b) { alpha_ = a; beta_ = b; return *this; }
   Gemm& aux(const double* p, i64 ld, i64 sb) { aux_ = p; ldaux = ld; sAuxb = sb; return *this; }
+  Gemm& transposed_copy(double* p, i64 ld, i64 sb) { ct_ = p; ldct = ld; sCtb = sb; return *this; }   // Ct_b[n][m] too
 };
 
 // tile configurations of dgemm_kernel
@@ -91,17 +93,27 @@ struct Gemm {
 #define THC_BIG_ST 4
 #endif
 #define THC_BIG 128, 128, THC_BIG_BK, 2, 4, THC_BIG_ST
+#define THC_MID 128, 64, 16, 4, 2, 4
 #define THC_SMALL 64, 64, 16, 2, 2, 4
 constexpr int BIG_THREADS = 256, SMALL_THREADS = 128;
 constexpr int gemm_smem_bytes(int BM, int BN, int BK, int ST, bool akm, bool bkm) {
   return ST * ((akm ? BM * BK : BK * (BM + 2)) + (bkm ? BN * BK : BK * (BN + 2))) * 8;
 }
+// tile 0: 128x128 (one CTA per SM), 1: 128x64 (two), 2: 64x64 (three)
+struct TileCfg { int BM, BN, per_sm; double lone_rate, pipe_share; };
+constexpr TileCfg TILE_CFGS[3] = {{128, 128, 1, 1.0, 1.0}, {128, 64, 2, 0.7, 0.9}, {64, 64, 3, 0.5, 0.75}};
 
 template <bool AKM, bool BKM, bool AL16>
-static cudaError_t launch_gemm_variant(bool big, dim3 grid, cudaStream_t st, const GemmParams& p) {
-  if (big) {
+static cudaError_t launch_gemm_variant(int tile, dim3 grid, cudaStream_t st, const GemmParams& p) {
+  if (tile == 0) {
     auto k = dgemm_kernel<THC_BIG, AKM, BKM, AL16>;
     int sm = gemm_smem_bytes(128, 128, THC_BIG_BK, THC_BIG_ST, AKM, BKM);
+    static bool done = false;
+    if (!done) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, sm); done = true; }
+    k<<<grid, BIG_THREADS, sm, st>>>(p);
+  } else if (tile == 1) {
+    auto k = dgemm_kernel<THC_MID, AKM, BKM, AL16>;
+    int sm = gemm_smem_bytes(128, 64, 16, 4, AKM, BKM);
     static bool done = false;
     if (!done) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, sm); done = true; }
     k<<<grid, BIG_THREADS, sm, st>>>(p);
@@ -157,28 +169,28 @@ struct Ctx {
   void gemm(const Gemm& g) {
     if (g.M <= 0 || g.N <= 0 || g.nbatch <= 0) return;
     // Tile shape and split-K factor: minimise  waves x (k-iterations per CTA + fixed cost) x tile area / tile rate  over
-    // {128x128 (1 CTA/SM), 64x64 (3 CTAs/SM)} x splits; a split-K pass adds a partial-tile write and a reduction.
+    // TILE_CFGS x splits; a split-K pass adds a partial-tile write and a reduction.
     const i64 kiters = (i64)g.nkb * ((g.K + 15) / 16);
-    bool big = false; int splits = 1; double best = 1e300;
-    for (int cfg = 0; cfg < 2; cfg++) {
-      const int T = cfg == 0 ? 128 : 64;
-      if (cfg == 0 && (g.M <= 64 || g.N <= 64)) continue;
-      const i64 tmn = (i64)((g.M + T - 1) / T) * ((g.N + T - 1) / T) * g.nbatch;
-      const double slots = (double)h->sms * (cfg == 0 ? 1 : 3);
-      const int smax = (int)std::max<i64>(1, std::min<i64>(64, kiters / 8));
+    int tile = 2, splits = 1; double best = 1e300;
+    for (int cfg = 0; cfg < 3; cfg++) {
+      const TileCfg& tc = TILE_CFGS[cfg];
+      if (cfg < 2 && (g.M <= 64 || g.N <= (cfg == 0 ? 64 : 32))) continue;
+      const i64 tmn = (i64)((g.M + tc.BM - 1) / tc.BM) * ((g.N + tc.BN - 1) / tc.BN) * g.nbatch;
+      const double slots = (double)h->sms * tc.per_sm;
+      const int smax = g.ct_ ? 1 : (int)std::max<i64>(1, std::min<i64>(64, kiters / 8));   // the transposed copy is written by the main kernel only
       for (int sp = 1; sp <= smax; sp++) {
         const double waves = std::ceil((double)tmn * sp / slots);
-        // per-CTA DMMA rate relative to a 128x128 CTA that owns an SM: a lone 64x64 CTA (one warp per sub-partition)
-        // reaches ~0.5, three of them share ~0.75 of the pipe
-        const double conc = std::min(3.0, std::ceil((double)tmn * sp / h->sms));
-        const double rate = cfg == 0 ? 1.0 : std::min(0.5, 0.75 / conc);
-        double t = waves * ((double)kiters / sp + 6.0) * T * T / rate;
+        // per-CTA DMMA rate relative to a 128x128 CTA that owns an SM: a lone smaller CTA cannot fill the pipe
+        // (lone_rate), several of them share pipe_share of it
+        const double conc = std::min((double)tc.per_sm, std::ceil((double)tmn * sp / h->sms));
+        const double rate = std::min(tc.lone_rate, tc.pipe_share / conc);
+        double t = waves * ((double)kiters / sp + 6.0) * tc.BM * tc.BN / rate;
         if (sp > 1) t += 0.025 * sp * (double)g.M * g.N * g.nbatch;     // partial-tile write + reduction at ~5 TB/s, same units
-        if (t < best * (sp > 1 ? 0.97 : 1.0)) { best = t; big = cfg == 0; splits = sp; }
+        if (t < best * (sp > 1 ? 0.97 : 1.0)) { best = t; tile = cfg; splits = sp; }
       }
     }
-    const int BMN = big ? 128 : 64;
-    const i64 tiles_mn = (i64)((g.M + BMN - 1) / BMN) * ((g.N + BMN - 1) / BMN);
+    const TileCfg& tc = TILE_CFGS[tile];
+    const i64 tiles_mn = (i64)((g.M + tc.BM - 1) / tc.BM) * ((g.N + tc.BN - 1) / tc.BN);
     const i64 per = (i64)g.nbatch * g.M * g.N;
     if (splits > 1) splitk_need = std::max(splitk_need, per * splits);
     if (dry || !ok()) return;
@@ -191,6 +203,7 @@ struct Ctx {
     p.batch = g.nbatch; p.sAb = g.sAb; p.sBb = g.sBb; p.sAuxb = g.sAuxb;
     p.kbatch = g.nkb; p.sAk = g.sAk; p.sBk = g.sBk;
     p.splits = splits; p.alpha = g.alpha_; p.beta = g.beta_;
+    p.Ct = g.ct_; p.ldct = g.ldct; p.sCtb = g.sCtb;
     if (splits > 1) { p.C = splitk; p.ldc = g.N; p.sCb = (i64)g.M * g.N; p.sCs = per; }
     else            { p.C = g.C; p.ldc = g.ldc; p.sCb = g.sCb; p.sCs = 0; }
 
@@ -203,19 +216,19 @@ struct Ctx {
     cudaError_t e;
     char desc[160];
     if (h->prof_mask & 1)
-      snprintf(desc, sizeof desc, "gemm %s M=%d N=%d K=%d batch=%d kbatch=%d splits=%d %c%c%s", big ? "big" : "small", g.M, g.N, g.K,
+      snprintf(desc, sizeof desc, "gemm %s M=%d N=%d K=%d batch=%d kbatch=%d splits=%d %c%c%s", tile == 0 ? "big" : (tile == 1 ? "mid" : "small"), g.M, g.N, g.K,
                g.nbatch, g.nkb, splits, g.akm ? 'K' : 'M', g.bkm ? 'K' : 'N', al16 ? "" : " unaligned");
     prof_start(0, desc, 2.0 * g.M * g.N * (double)g.K * g.nbatch * g.nkb);
     const int sel = (g.akm ? 4 : 0) | (g.bkm ? 2 : 0) | (al16 ? 1 : 0);
     switch (sel) {
-      case 7: e = launch_gemm_variant<true, true, true>(big, grid, h->stream, p); break;
-      case 6: e = launch_gemm_variant<true, true, false>(big, grid, h->stream, p); break;
-      case 5: e = launch_gemm_variant<true, false, true>(big, grid, h->stream, p); break;
-      case 4: e = launch_gemm_variant<true, false, false>(big, grid, h->stream, p); break;
-      case 3: e = launch_gemm_variant<false, true, true>(big, grid, h->stream, p); break;
-      case 2: e = launch_gemm_variant<false, true, false>(big, grid, h->stream, p); break;
-      case 1: e = launch_gemm_variant<false, false, true>(big, grid, h->stream, p); break;
-      default: e = launch_gemm_variant<false, false, false>(big, grid, h->stream, p); break;
+      case 7: e = launch_gemm_variant<true, true, true>(tile, grid, h->stream, p); break;
+      case 6: e = launch_gemm_variant<true, true, false>(tile, grid, h->stream, p); break;
+      case 5: e = launch_gemm_variant<true, false, true>(tile, grid, h->stream, p); break;
+      case 4: e = launch_gemm_variant<true, false, false>(tile, grid, h->stream, p); break;
+      case 3: e = launch_gemm_variant<false, true, true>(tile, grid, h->stream, p); break;
+      case 2: e = launch_gemm_variant<false, true, false>(tile, grid, h->stream, p); break;
+      case 1: e = launch_gemm_variant<false, false, true>(tile, grid, h->stream, p); break;
+      default: e = launch_gemm_variant<false, false, false>(tile, grid, h->stream, p); break;
     }
     h->launches++;
     check(e);
@@ -262,14 +275,19 @@ struct Ctx {
     THC_EW(combine_kernel, np2, 8.0 * np2 * (3.0 * nl + 4.0), Mo, Mv, omat, vmat, C3, np2, (int)nl);
   }
   void rowdot(const double* X, i64 ldx, const double* T, i64 sTb, i64 ldT, double* out, i64 ldo, i64 nb, i64 nr, i64 n) {
-    THC_EW(rowdot_kernel, nb * nr, 8.0 * ((double)nb * nr * n + (double)nr * n + (double)nb * nr), X, ldx, T, sTb, ldT, out, ldo, (int)nb, (int)nr, (int)n);
+    THC_EW(rowdot_kernel, nb * nr * 8 /* eight lanes per row */, 8.0 * ((double)nb * nr * n + (double)nr * n + (double)nb * nr), X, ldx, T, sTb, ldT, out, ldo, (int)nb, (int)nr, (int)n);
   }
   void coldot(const double* X, i64 ldx, const double* T, i64 sTb, i64 ldT, double* out, i64 ldo, i64 nb, i64 nc, i64 n) {
     THC_EW(coldot_kernel, nb * nc, 8.0 * ((double)nb * nc * n + (double)nc * n + (double)nb * nc), X, ldx, T, sTb, ldT, out, ldo, (int)nb, (int)nc, (int)n);
   }
   void rowscale(const double* X, i64 ldx, const double* Mrow, i64 ldm, const double* add, double alpha, double* out,
                 i64 nb, i64 n, i64 nc) {
-    THC_EW(rowscale_kernel, nb * n * nc, 8.0 * ((double)nb * n * nc * (add ? 2.0 : 1.0) + (double)n * nc + (double)nb * nc), X, ldx, Mrow, ldm, add, alpha, out, (int)nb, (int)n, (int)nc);
+    const double bytes = 8.0 * ((double)nb * n * nc * (add ? 2.0 : 1.0) + (double)n * nc + (double)nb * nc);
+    const bool vec = ((nc | ldx | ldm) & 1) == 0 &&
+                     ((reinterpret_cast<uintptr_t>(X) | reinterpret_cast<uintptr_t>(Mrow) | reinterpret_cast<uintptr_t>(add) |
+                       reinterpret_cast<uintptr_t>(out)) & 15) == 0;
+    if (vec) THC_EW(rowscale2_kernel, nb * n * nc / 2, bytes, X, ldx, Mrow, ldm, add, alpha, out, (int)nb, (int)n, (int)nc);
+    else THC_EW(rowscale_kernel, nb * n * nc, bytes, X, ldx, Mrow, ldm, add, alpha, out, (int)nb, (int)n, (int)nc);
   }
   void rowscale_inplace(double* T, const double* Mrow, i64 ldm, double alpha, i64 nb, i64 n, i64 nc) {
     THC_EW(rowscale_inplace_kernel, nb * n * nc, 8.0 * (2.0 * nb * n * nc + (double)nb * nc), T, Mrow, ldm, alpha, (int)nb, (int)n, (int)nc);
@@ -403,7 +421,7 @@ struct Ctx {
     }
     const cuuint64_t dims[3] = {(cuuint64_t)d0, (cuuint64_t)d1, (cuuint64_t)d2};
     const cuuint64_t strides[2] = {(cuuint64_t)d0 * 8, (cuuint64_t)d0 * (cuuint64_t)d1 * 8};
-    const cuuint32_t box[3] = {16, 16, 1}, es[3] = {1, 1, 1};
+    const cuuint32_t box[3] = {16, 16, (cuuint32_t)TP_IC}, es[3] = {1, 1, 1};
     CUresult r = reinterpret_cast<EncodeFn>(h->encode_tiled)(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<double*>(base), dims,
                                                              strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                                                              CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);

@@ -64,16 +64,28 @@ __global__ void combine_kernel(double* __restrict__ Mo, const double* __restrict
 }
 
 // out[b*ldo + r] = sum_{i<n} X[r*ldx + i] * T[b*sTb + r*ldT + i]      (a^L_P: Alg.2 l.541, Alg.8 l.788; C7: Alg.7 line 9 l.749)
+// Eight lanes share a row (lane j takes i = j, j + 8, ...: 64-byte coalesced segments), xor-shuffle reduction.
 __global__ void rowdot_kernel(const double* __restrict__ X, i64 ldx, const double* __restrict__ T, i64 sTb, i64 ldT,
                               double* __restrict__ out, i64 ldo, int nb, int nr, int n) {
-  i64 total = (i64)nb * nr;
-  THC_GRID_STRIDE(idx, total) {
-    int r = (int)(idx % nr), b = (int)(idx / nr);
-    const double* x = X + (i64)r * ldx;
-    const double* tt = T + (i64)b * sTb + (i64)r * ldT;
+  const i64 total = (i64)nb * nr;
+  const int sub = threadIdx.x & 7;
+  const i64 rows_per_pass = (i64)gridDim.x * (blockDim.x >> 3);
+  const i64 passes = (total + rows_per_pass - 1) / rows_per_pass;      // every lane runs every pass (full-warp shuffles)
+  i64 idx = (i64)blockIdx.x * (blockDim.x >> 3) + (threadIdx.x >> 3);
+  for (i64 it = 0; it < passes; it++, idx += rows_per_pass) {
     double s = 0.0;
-    for (int i = 0; i < n; i++) s = fma(x[i], tt[i], s);
-    out[(i64)b * ldo + r] = s;
+    const bool ok = idx < total;
+    int r = 0, b = 0;
+    if (ok) {
+      r = (int)(idx % nr); b = (int)(idx / nr);
+      const double* x = X + (i64)r * ldx;
+      const double* tt = T + (i64)b * sTb + (i64)r * ldT;
+      for (int i = sub; i < n; i += 8) s = fma(x[i], tt[i], s);
+    }
+    s += __shfl_xor_sync(0xffffffffu, s, 1);
+    s += __shfl_xor_sync(0xffffffffu, s, 2);
+    s += __shfl_xor_sync(0xffffffffu, s, 4);
+    if (ok && sub == 0) out[(i64)b * ldo + r] = s;
   }
 }
 
@@ -103,6 +115,23 @@ __global__ void rowscale_kernel(const double* __restrict__ X, i64 ldx, const dou
     double val = alpha * X[(i64)i * ldx + c] * Mrow[(i64)b * ldm + c];
     if (add) val += add[idx];
     out[idx] = val;
+  }
+}
+
+// the same, two columns per thread with 16-byte accesses (nc, ldx, ldm even; all pointers 16-byte aligned)
+__global__ void rowscale2_kernel(const double* __restrict__ X, i64 ldx, const double* __restrict__ Mrow, i64 ldm,
+                                 const double* __restrict__ add, double alpha, double* __restrict__ out, int nb, int n, int nc) {
+  const int nc2 = nc >> 1;
+  const i64 total = (i64)nb * n * nc2;
+  THC_GRID_STRIDE(idx, total) {
+    const int c = (int)(idx % nc2) * 2;
+    const i64 r = idx / nc2;
+    const int i = (int)(r % n), b = (int)(r / n);
+    const double2 x = *reinterpret_cast<const double2*>(X + (i64)i * ldx + c);
+    const double2 m = *reinterpret_cast<const double2*>(Mrow + (i64)b * ldm + c);
+    double2 val = make_double2(alpha * x.x * m.x, alpha * x.y * m.y);
+    if (add) { const double2 a = *reinterpret_cast<const double2*>(add + 2 * idx); val.x += a.x; val.y += a.y; }
+    *reinterpret_cast<double2*>(out + 2 * idx) = val;
   }
 }
 
@@ -197,11 +226,20 @@ __global__ void dot_partial_kernel(const double* __restrict__ a, const double* _
   if (threadIdx.x == 0) partial[blockIdx.x] = s;
 }
 
-// partial[block] = sum over a 32x32 tile pair of Z[P][Q] * E[l][P][Q] * E[l][Q][P]; grid = (tiles, tiles, nl), block (32, 8)
+// partial[block] = sum over the 32x32 tile pair {(bx,by), (by,bx)} of Z[P][Q] * E[l][P][Q] * E[l][Q][P].  Z is symmetric
+// (thc.h), so the two tiles of a pair contribute the same amount: only blocks with bx <= by work (each reads both
+// tiles once -- E is streamed exactly once overall) and off-diagonal pairs count twice; blocks with bx > by write 0.
+// grid = (tiles, tiles, nl), block (32, 8).
 __global__ void zee_partial_kernel(const double* __restrict__ Z, const double* __restrict__ E, int NP, double* __restrict__ partial) {
   __shared__ double tile[32][33];
+  __shared__ double sh[8];
+  const int bx = blockIdx.x, by = blockIdx.y;
+  const i64 slot = ((i64)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+  if (bx > by) {
+    if (threadIdx.x == 0 && threadIdx.y == 0) partial[slot] = 0.0;
+    return;
+  }
   const double* El = E + (i64)blockIdx.z * NP * NP;
-  int bx = blockIdx.x, by = blockIdx.y;
   for (int j = threadIdx.y; j < 32; j += blockDim.y) {
     int r = bx * 32 + j, c = by * 32 + threadIdx.x;
     tile[j][threadIdx.x] = (r < NP && c < NP) ? El[(i64)r * NP + c] : 0.0;
@@ -212,15 +250,14 @@ __global__ void zee_partial_kernel(const double* __restrict__ Z, const double* _
     int r = by * 32 + j, c = bx * 32 + threadIdx.x;
     if (r < NP && c < NP) s = fma(Z[(i64)r * NP + c] * El[(i64)r * NP + c], tile[threadIdx.x][j], s);
   }
-  // block reduction over 256 threads (blockDim = 32 x 8)
-  __shared__ double sh[8];
+  if (bx != by) s *= 2.0;
   for (int off = 16; off > 0; off >>= 1) s += __shfl_down_sync(0xffffffffu, s, off);
   if (threadIdx.x == 0) sh[threadIdx.y] = s;
   __syncthreads();
   if (threadIdx.x == 0 && threadIdx.y == 0) {
     double tot = 0.0;
     for (int k = 0; k < (int)blockDim.y; k++) tot += sh[k];
-    partial[((i64)blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x] = tot;
+    partial[slot] = tot;
   }
 }
 

@@ -305,9 +305,8 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out, const Shard& sh
         c.gemm(Gemm(VY, NX, 'K', Yv, NX, 'K', BI, v, ni * o, v, NX));
         // line 10: G_I[q][r] = sum_ia Xo[i,q] Xv[a,r] BI[I][i][a]
         c.gemm(Gemm(XvT, v, 'K', BI, v, 'K', GXT, o, NP, o, v).batch(ni, 0, ov, NP * o));
-        c.gemm(Gemm(XoT, o, 'K', GXT, o, 'K', Gt, NPp, NP, NP, o).batch(ni, 0, NP * o, NPp * NPp));
-        // and its transpose GtT_I[q][r] = G_I[r][q] (operands swapped), read by the mirrored half of line 11
-        c.gemm(Gemm(GXT, o, 'K', XoT, o, 'K', GtT, NPp, NP, NP, o).batch(ni, NP * o, 0, NPp * NPp));
+        // (the epilogue also writes the transpose GtT_I[q][r] = G_I[r][q], read by the mirrored half of line 11)
+        c.gemm(Gemm(XoT, o, 'K', GXT, o, 'K', Gt, NPp, NP, NP, o).batch(ni, 0, NP * o, NPp * NPp).transposed_copy(GtT, NPp, NPp * NPp));
         // lines 8-9: E_I[p][q] = sum_i Cc[p][(q,i)] Yo[i,I] ;  F_I[p][r] = sum_a Dd[p][(r,a)] Yv[a,I]
         c.gemm(Gemm(YoT + I0 * o, o, 'K', Cc, o, 'K', Eb, bXp * NPp, ni, NP, o).batch(npb, 0, NP * o, NPp));
         c.gemm(Gemm(YvT + I0 * v, v, 'K', Dd, v, 'K', Fb, bXp * NPp, ni, NP, v).batch(npb, 0, NP * v, NPp));
@@ -522,7 +521,34 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
     if (!fix_bP7) h->bP7 = 1;
     if (!fix_bI) h->bI = std::min<int64_t>(NX, 16);
     while (!fix_bL && h->bL > 1 && need_device(h) > cap) h->bL = h->bL / 2;
-    h->bX = sX; h->bP7 = sP; h->bI = sI;
+    // stage B: the Alg.7 phase on its own
+    h->bP7 = sP;
+    while (!fix_bP7 && h->bP7 > 1 && need_device(h) > cap) h->bP7 = h->bP7 / 2;
+    // stage C: Alg.6.  H[bX][NPp][NPp] and the G_I chunk (bI grid points, both orientations) compete for the same
+    // memory: every row block recomputes all G_I (cost ~ 1/bX), every chunk reads and rewrites H (cost ~ 1/bI).  Take
+    // the (bX, bI) pair that minimises  ceil(NP/bX) * t(G pass) + ceil(NX/bI) * t(H read + write)  among those that fit.
+    h->bX = sX; h->bI = sI;
+    if (!fix_bX && !fix_bI && need_device(h) > cap) {
+      const double fo = (double)o, fv = (double)v, fNP = (double)NP, fNX = (double)NX;
+      const double t_g = fNX * (2 * fo * fv * fNP + 2 * fo * fNP * fNP + 2 * fo * fv * fNX) / 25e12;       // DMMA, s
+      const double t_h = 16.0 * fNP * (double)pad_to(NP, 32) * (double)pad_to(NP, 32) / 5e12;            // HBM, s
+      double best = 1e300; int64_t bestX = 0, bestI = 0;
+      for (int64_t bi : {16, 24, 32, 48, 64, 96, 128, 192, 256, 384, 512}) {
+        if (bi > NX) break;
+        h->bI = bi; h->bX = 16;
+        if (need_device(h) > cap) break;
+        int64_t lo = 1, hi = pad_to(NP, 16) / 16;              // largest bX = 16 * lo that fits
+        while (lo < hi) {
+          const int64_t mid = (lo + hi + 1) / 2;
+          h->bX = 16 * mid;
+          if (need_device(h) <= cap) lo = mid; else hi = mid - 1;
+        }
+        const int64_t bx = 16 * lo;
+        const double t = std::ceil(fNP / (double)bx) * t_g + std::ceil(fNX / (double)bi) * t_h;
+        if (t < best) { best = t; bestX = bx; bestI = bi; }
+      }
+      if (bestX) { h->bX = bestX; h->bI = bestI; } else { h->bX = sX; h->bI = sI; }
+    }
   }
   for (;;) {
     h->need_bytes = need_device(h);

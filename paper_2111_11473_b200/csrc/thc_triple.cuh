@@ -28,8 +28,10 @@
 namespace thc {
 
 constexpr int TP_PT = 16, TP_QT = 16, TP_RT = 32;
-constexpr int TP_STAGES = 8, TP_LOOKAHEAD = TP_STAGES - 2;
-constexpr int TP_BLK_BYTES = 16 * 16 * 8;                  // one 16x16 FP64 block
+constexpr int TP_IC = 2;                                   // grid points per pipeline stage (one barrier round-trip per stage)
+constexpr int TP_STAGES = 5, TP_LOOKAHEAD = TP_STAGES - 2;
+constexpr int TP_SLICE_BYTES = 16 * 16 * 8;                // one 16x16 FP64 block of one grid point
+constexpr int TP_BLK_BYTES = TP_IC * TP_SLICE_BYTES;       // one TMA box: 16 x 16 x TP_IC
 constexpr int TP_STAGE_BYTES = 10 * TP_BLK_BYTES;          // EPQ FPQ EPR0 EPR1 FPR0 FPR1 GQR0 GQR1 GTQR0 GTQR1
 constexpr int TP_SMEM_BYTES = TP_STAGES * TP_STAGE_BYTES + 1024 /* alignment slack */ + 2 * TP_STAGES * 8;
 constexpr int TP_THREADS = 256;
@@ -73,8 +75,43 @@ __device__ __forceinline__ double2 lds128(const uint8_t* base, uint32_t off) {
   return *reinterpret_cast<const double2*>(base + off);
 }
 
+
+// One grid point of the register-tile update.  `sl` = the grid point's slice inside the stage (block b of the stage at
+// sl + b * TP_BLK_BYTES).  hrq[a][b][c] accumulates H[p_a][r_c][q_b].
+template <bool DIAG>
+__device__ __forceinline__ void tp_update(const uint8_t* sl, const uint32_t (&offPQ)[4], const uint32_t (&offPR)[4],
+                                          const uint32_t (&offQR)[2], double (&hqr)[4][2][4], double (&hrq)[4][2][4]) {
+  double gqr[2][4], gt[2][4];            // gt[b][c] = G_I[r_c][q_b] (read from the transposed copy GT_I[q][r])
+#pragma unroll
+  for (int b = 0; b < 2; b++) {
+    double2 g0 = lds128(sl, offQR[b]), g1 = lds128(sl, (offQR[b] ^ 64));
+    gqr[b][0] = g0.x; gqr[b][1] = g0.y; gqr[b][2] = g1.x; gqr[b][3] = g1.y;
+    if (!DIAG) {
+      double2 h0 = lds128(sl, 2 * TP_BLK_BYTES + offQR[b]), h1 = lds128(sl, 2 * TP_BLK_BYTES + (offQR[b] ^ 64));
+      gt[b][0] = h0.x; gt[b][1] = h0.y; gt[b][2] = h1.x; gt[b][3] = h1.y;
+    }
+  }
+#pragma unroll
+  for (int a = 0; a < 4; a++) {
+    double2 e = lds128(sl, offPQ[a]), f = lds128(sl, TP_BLK_BYTES + offPQ[a]);
+    double2 e0 = lds128(sl, offPR[a]), e1 = lds128(sl, (offPR[a] ^ 64));
+    double2 f0 = lds128(sl, 2 * TP_BLK_BYTES + offPR[a]), f1 = lds128(sl, 2 * TP_BLK_BYTES + (offPR[a] ^ 64));
+    const double epq[2] = {e.x, e.y}, fpq[2] = {f.x, f.y};
+    const double epr[4] = {e0.x, e0.y, e1.x, e1.y}, fpr[4] = {f0.x, f0.y, f1.x, f1.y};
+#pragma unroll
+    for (int b = 0; b < 2; b++)
+#pragma unroll
+      for (int c = 0; c < 4; c++) {
+        const double sv = fma(epr[c], fpq[b], epq[b] * fpr[c]);
+        hqr[a][b][c] = fma(sv, gqr[b][c], hqr[a][b][c]);
+        if (!DIAG) hrq[a][b][c] = fma(sv, gt[b][c], hrq[a][b][c]);
+      }
+  }
+}
+
 // E, F: tensor maps over [nI][nPp][NPp] (innermost NPp); G, GT: over [nI][NPp][NPp] with GT_I[q][r] = G_I[r][q] (so that the
-// mirrored block is read with the same row-q / chunk-r pattern as the direct one); box 16 x 16 x 1, SWIZZLE_128B.
+// mirrored block is read with the same row-q / chunk-r pattern as the direct one); box 16 x 16 x TP_IC, SWIZZLE_128B.
+// Grid points beyond nI (odd nI) are zero-filled by the TMA unit and add nothing.
 __global__ void __launch_bounds__(TP_THREADS, 1)
 triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_constant__ CUtensorMap mapF,
                       const __grid_constant__ CUtensorMap mapG, const __grid_constant__ CUtensorMap mapGT,
@@ -94,7 +131,8 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
   // r: this thread owns r = wr*16 + {2 lr, 2 lr + 1, 2 lr + 8, 2 lr + 9}  -> block wr, chunks lr and lr + 4
 
   const int my_items = p.n_items > (int)blockIdx.x ? (p.n_items - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
-  const int total = my_items * p.nI;          // < 2^31 (checked by the launcher)
+  const int nS = (p.nI + TP_IC - 1) / TP_IC;            // stages per work item
+  const int total = my_items * nS;                      // < 2^31 (checked by the launcher)
 
   if (tid == 0) {
     for (int s = 0; s < TP_STAGES; s++) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, 8); }
@@ -102,10 +140,16 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
   }
   __syncthreads();
 
-  // ---- producer side (lane 0 of each warp takes every 8th iteration) -------------------------------------------------
-  auto issue = [&](int jn, int k, int I) {          // fill for flat iteration jn = (item k of this CTA, grid point I)
-    const TripleItem it = p.items[blockIdx.x + (long long)k * gridDim.x];
-    const int s = jn % TP_STAGES;
+  // ---- producer (thread 0 only): flat fill index pj = (item pk of this CTA, stage pS of the item) ------------------------
+  // (its counters live in shared memory: the compute loop needs every register of the 255-register budget)
+  __shared__ int prod[3];
+  if (tid == 0) { prod[0] = 0; prod[1] = 0; prod[2] = 0; }
+  auto fill = [&]() {
+    int pj = prod[0], pk = prod[1], pS = prod[2];
+    if (pj >= total) return;
+    const TripleItem it = p.items[blockIdx.x + (long long)pk * gridDim.x];
+    const int s = pj % TP_STAGES, f = pj / TP_STAGES, I = pS * TP_IC;
+    if (f > 0) mbar_wait(bar_empty + 8 * s, (uint32_t)((f - 1) & 1));
     const uint32_t dst = ring + s * TP_STAGE_BYTES, bf = bar_full + 8 * s;
     mbar_expect_tx(bf, it.diag ? 8 * TP_BLK_BYTES : 10 * TP_BLK_BYTES);
     tma_load_3d(dst + 0 * TP_BLK_BYTES, &mapE, it.q0, it.p0, I, bf);
@@ -120,19 +164,14 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
       tma_load_3d(dst + 8 * TP_BLK_BYTES, &mapGT, it.r0, it.q0, I, bf);
       tma_load_3d(dst + 9 * TP_BLK_BYTES, &mapGT, it.r0 + 16, it.q0, I, bf);
     }
+    pj++;
+    if (++pS == nS) { pS = 0; pk++; }
+    prod[0] = pj; prod[1] = pk; prod[2] = pS;
   };
-  if (tid == 0) {
-    int k = 0, I = 0;
-    for (int jn = 0; jn < TP_LOOKAHEAD && jn < total; jn++) {
-      issue(jn, k, I);
-      if (++I == p.nI) { I = 0; k++; }
-    }
-  }
-  // this warp refills iterations jn = warp + TP_LOOKAHEAD + 8 m
-  int pj = warp + TP_LOOKAHEAD;
-  int pk = pj / p.nI, pI = pj % p.nI;
+  if (tid == 0)
+    for (int n = 0; n < TP_LOOKAHEAD; n++) fill();
 
-  // ---- per-thread shared-memory byte offsets inside a stage (swizzle: chunk ^= row & 7) ------------------------------
+  // ---- per-thread shared-memory byte offsets inside a grid point's slice (swizzle: chunk ^= row & 7) -------------------
   uint32_t offPQ[4], offPR[4], offQR[2];
 #pragma unroll
   for (int a = 0; a < 4; a++) {
@@ -146,114 +185,61 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
     offQR[b] = (6 + wr) * TP_BLK_BYTES + row * 128 + ((lr ^ (row & 7)) << 4);
   }
 
-  double hqr[4][2][4], hrq[4][2][4];      // hrq[a][b][c] accumulates H[p_a][r_c][q_b]
-  int I = 0, k = 0;
-  TripleItem cur = my_items > 0 ? p.items[blockIdx.x] : TripleItem{0, 0, 0, 1};
+  double hqr[4][2][4], hrq[4][2][4];
+  int st = 0;                 // ring stage of the current iteration
+  uint32_t par = 0;           // its mbarrier phase parity
+  for (int k = 0; k < my_items; k++) {
+    const int diag = p.items[blockIdx.x + (long long)k * gridDim.x].diag;
+#pragma unroll
+    for (int a = 0; a < 4; a++)
+#pragma unroll
+      for (int b = 0; b < 2; b++)
+#pragma unroll
+        for (int c = 0; c < 4; c++) hqr[a][b][c] = hrq[a][b][c] = 0.0;
 
-  for (int j = 0; j < total; j++) {
-    if (I == 0) {
-#pragma unroll
-      for (int a = 0; a < 4; a++)
-#pragma unroll
-        for (int b = 0; b < 2; b++)
-#pragma unroll
-          for (int c = 0; c < 4; c++) hqr[a][b][c] = hrq[a][b][c] = 0.0;
-    }
-    const int s = j % TP_STAGES;
-    const uint32_t par = (uint32_t)((j / TP_STAGES) & 1);
-    mbar_wait(bar_full + 8 * s, par);
-
-    // refill (two iterations behind the consumers)
-    if ((j & 7) == warp) {
-      if (lane == 0 && pj < total) {
-        const int sn = pj % TP_STAGES;
-        const int fill = pj / TP_STAGES;
-        if (fill > 0) mbar_wait(bar_empty + 8 * sn, (uint32_t)((fill - 1) & 1));
-        issue(pj, pk, pI);
-      }
-      pj += 8; pI += 8;
-      while (pI >= p.nI) { pI -= p.nI; pk++; }
+    for (int s = 0; s < nS; s++) {
+      mbar_wait(bar_full + 8 * st, par);
+      if (tid == 0) fill();                          // TP_LOOKAHEAD stages ahead, two iterations behind the consumers
       __syncwarp();
+      const uint8_t* sl = ring_ptr + st * TP_STAGE_BYTES;
+      if (diag) {
+#pragma unroll 1
+        for (int ii = 0; ii < TP_IC; ii++) tp_update<true>(sl + ii * TP_SLICE_BYTES, offPQ, offPR, offQR, hqr, hrq);
+      } else {
+#pragma unroll 1
+        for (int ii = 0; ii < TP_IC; ii++) tp_update<false>(sl + ii * TP_SLICE_BYTES, offPQ, offPR, offQR, hqr, hrq);
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar_empty + 8 * st);
+      if (++st == TP_STAGES) { st = 0; par ^= 1; }
     }
 
-    const uint8_t* st = ring_ptr + s * TP_STAGE_BYTES;
-    double gqr[2][4], gt[2][4];            // gt[b][c] = G_I[r_c][q_b] (read from the transposed copy GT_I[q][r])
+    // ---- write back this item's block(s) of H[p][q][r] ---------------------------------------------------------------
+    const TripleItem cur = p.items[blockIdx.x + (long long)k * gridDim.x];
+    const long long sHp = (long long)p.NPp * p.NPp;
+    const int rA = cur.r0 + wr * 16 + 2 * lr;              // r = rA, rA + 1, rA + 8, rA + 9
 #pragma unroll
-    for (int b = 0; b < 2; b++) {
-      double2 g0 = lds128(st, offQR[b]), g1 = lds128(st, (offQR[b] ^ 64));
-      gqr[b][0] = g0.x; gqr[b][1] = g0.y; gqr[b][2] = g1.x; gqr[b][3] = g1.y;
-    }
-    if (!cur.diag) {
+    for (int a = 0; a < 4; a++) {
+      double* Hp = p.H + (long long)(cur.p0 + tp0 + a) * sHp;
 #pragma unroll
       for (int b = 0; b < 2; b++) {
-        double2 g0 = lds128(st, 2 * TP_BLK_BYTES + offQR[b]), g1 = lds128(st, 2 * TP_BLK_BYTES + (offQR[b] ^ 64));
-        gt[b][0] = g0.x; gt[b][1] = g0.y; gt[b][2] = g1.x; gt[b][3] = g1.y;
+        double* row = Hp + (long long)(cur.q0 + tq0 + b) * p.NPp;
+        double2* d0 = reinterpret_cast<double2*>(row + rA);
+        double2* d1 = reinterpret_cast<double2*>(row + rA + 8);
+        double2 v0 = make_double2(hqr[a][b][0], hqr[a][b][1]), v1 = make_double2(hqr[a][b][2], hqr[a][b][3]);
+        if (p.accumulate) { double2 o0 = *d0, o1 = *d1; v0.x += o0.x; v0.y += o0.y; v1.x += o1.x; v1.y += o1.y; }
+        *d0 = v0; *d1 = v1;
       }
+      if (!cur.diag) {
 #pragma unroll
-      for (int a = 0; a < 4; a++) {
-        double2 e = lds128(st, offPQ[a]), f = lds128(st, TP_BLK_BYTES + offPQ[a]);
-        double2 e0 = lds128(st, offPR[a]), e1 = lds128(st, (offPR[a] ^ 64));
-        double2 f0 = lds128(st, 2 * TP_BLK_BYTES + offPR[a]), f1 = lds128(st, 2 * TP_BLK_BYTES + (offPR[a] ^ 64));
-        const double epq[2] = {e.x, e.y}, fpq[2] = {f.x, f.y};
-        const double epr[4] = {e0.x, e0.y, e1.x, e1.y}, fpr[4] = {f0.x, f0.y, f1.x, f1.y};
-#pragma unroll
-        for (int b = 0; b < 2; b++)
-#pragma unroll
-          for (int c = 0; c < 4; c++) {
-            const double sv = fma(epr[c], fpq[b], epq[b] * fpr[c]);
-            hqr[a][b][c] = fma(sv, gqr[b][c], hqr[a][b][c]);
-            hrq[a][b][c] = fma(sv, gt[b][c], hrq[a][b][c]);
-          }
-      }
-    } else {
-#pragma unroll
-      for (int a = 0; a < 4; a++) {
-        double2 e = lds128(st, offPQ[a]), f = lds128(st, TP_BLK_BYTES + offPQ[a]);
-        double2 e0 = lds128(st, offPR[a]), e1 = lds128(st, (offPR[a] ^ 64));
-        double2 f0 = lds128(st, 2 * TP_BLK_BYTES + offPR[a]), f1 = lds128(st, 2 * TP_BLK_BYTES + (offPR[a] ^ 64));
-        const double epq[2] = {e.x, e.y}, fpq[2] = {f.x, f.y};
-        const double epr[4] = {e0.x, e0.y, e1.x, e1.y}, fpr[4] = {f0.x, f0.y, f1.x, f1.y};
-#pragma unroll
-        for (int b = 0; b < 2; b++)
-#pragma unroll
-          for (int c = 0; c < 4; c++) {
-            const double sv = fma(epr[c], fpq[b], epq[b] * fpr[c]);
-            hqr[a][b][c] = fma(sv, gqr[b][c], hqr[a][b][c]);
-          }
-      }
-    }
-    __syncwarp();
-    if (lane == 0) mbar_arrive(bar_empty + 8 * s);
-
-    if (++I == p.nI) {
-      // ---- write back this item's block(s) of H[p][q][r] -----------------------------------------------------------
-      const long long sHp = (long long)p.NPp * p.NPp;
-      const int rA = cur.r0 + wr * 16 + 2 * lr;              // r = rA, rA + 1, rA + 8, rA + 9
-#pragma unroll
-      for (int a = 0; a < 4; a++) {
-        double* Hp = p.H + (long long)(cur.p0 + tp0 + a) * sHp;
-#pragma unroll
-        for (int b = 0; b < 2; b++) {
-          double* row = Hp + (long long)(cur.q0 + tq0 + b) * p.NPp;
-          double2* d0 = reinterpret_cast<double2*>(row + rA);
-          double2* d1 = reinterpret_cast<double2*>(row + rA + 8);
-          double2 v0 = make_double2(hqr[a][b][0], hqr[a][b][1]), v1 = make_double2(hqr[a][b][2], hqr[a][b][3]);
-          if (p.accumulate) { double2 o0 = *d0, o1 = *d1; v0.x += o0.x; v0.y += o0.y; v1.x += o1.x; v1.y += o1.y; }
-          *d0 = v0; *d1 = v1;
-        }
-        if (!cur.diag) {
-#pragma unroll
-          for (int c = 0; c < 4; c++) {
-            const int r = rA + (c & 1) + 8 * (c >> 1);
-            double2* d = reinterpret_cast<double2*>(Hp + (long long)r * p.NPp + cur.q0 + tq0);
-            double2 vv = make_double2(hrq[a][0][c], hrq[a][1][c]);
-            if (p.accumulate) { double2 o = *d; vv.x += o.x; vv.y += o.y; }
-            *d = vv;
-          }
+        for (int c = 0; c < 4; c++) {
+          const int r = rA + (c & 1) + 8 * (c >> 1);
+          double2* d = reinterpret_cast<double2*>(Hp + (long long)r * p.NPp + cur.q0 + tq0);
+          double2 vv = make_double2(hrq[a][0][c], hrq[a][1][c]);
+          if (p.accumulate) { double2 o = *d; vv.x += o.x; vv.y += o.y; }
+          *d = vv;
         }
       }
-      I = 0; k++;
-      if (k < my_items) cur = p.items[blockIdx.x + (long long)k * gridDim.x];
     }
   }
 }
