@@ -29,16 +29,10 @@ namespace thc {
 
 constexpr int TP_PT = 16, TP_QT = 16, TP_RT = 32;
 constexpr int TP_IC = 2;                                   // grid points per pipeline stage (one barrier round-trip per stage)
-constexpr int TP_STAGES = 4, TP_LOOKAHEAD = TP_STAGES - 2;
-constexpr int TP_BLK = 16 * 16 * 8;                        // one 16x16 FP64 block of one grid point (2 KB)
-// slice of one grid point: E blocks and G blocks in 2 KB slots, F blocks in 3 KB slots with the data 512 B into the
-// slot: the 128-byte swizzle is a function of the shared-memory address, so F rows land in the other 64-byte half of
-// the banks than the E rows of the same (p, column) and an E/F fragment pair is read without bank conflicts
-constexpr int TP_OFF_EPQ = 0, TP_OFF_EPR0 = 2048, TP_OFF_EPR1 = 4096;
-constexpr int TP_OFF_GQR0 = 6144, TP_OFF_GQR1 = 8192, TP_OFF_GTQR0 = 10240, TP_OFF_GTQR1 = 12288;
-constexpr int TP_OFF_FPQ = 14336 + 512, TP_OFF_FPR0 = 17408 + 512, TP_OFF_FPR1 = 20480 + 512;
-constexpr int TP_SLICE_BYTES = 23552;                      // 7 x 2 KB + 3 x 3 KB
-constexpr int TP_STAGE_BYTES = TP_IC * TP_SLICE_BYTES;
+constexpr int TP_STAGES = 5, TP_LOOKAHEAD = TP_STAGES - 2;
+constexpr int TP_SLICE_BYTES = 16 * 16 * 8;                // one 16x16 FP64 block of one grid point
+constexpr int TP_BLK_BYTES = TP_IC * TP_SLICE_BYTES;       // one TMA box: 16 x 16 x TP_IC
+constexpr int TP_STAGE_BYTES = 10 * TP_BLK_BYTES;          // EPQ FPQ EPR0 EPR1 FPR0 FPR1 GQR0 GQR1 GTQR0 GTQR1
 constexpr int TP_SMEM_BYTES = TP_STAGES * TP_STAGE_BYTES + 1024 /* alignment slack */ + 2 * TP_STAGES * 8;
 constexpr int TP_THREADS = 256;
 
@@ -82,46 +76,41 @@ __device__ __forceinline__ double2 lds128(const uint8_t* base, uint32_t off) {
 }
 
 
-__device__ __forceinline__ double lds64(const uint8_t* base, uint32_t off) {
-  return *reinterpret_cast<const double*>(base + off);
-}
-__device__ __forceinline__ void dmma884_tp(double& d0, double& d1, double a, double b) {
-  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-               : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
-}
-
-// One grid point.  The bracket s_I[p](q,r) = E_pq F_pr + F_pq E_pr is a rank-2 outer product over (q, r): one
-// DMMA.8x8x4 with A = [E_pq  F_pq  0  0] (rows q) and B = [F_pr; E_pr; 0; 0] (columns r) forms it for an 8 x 8 block of
-// (q, r) and leaves, in lane (g, t), s[q = pi(g)][r = 2t, 2t+1] -- next to the G values of the same (q, r), which do not
-// depend on p and stay in registers for all 16 p.  Two of the four k of the DMMA are idle, which costs pipe time
-// (16 clk per 64 brackets instead of 8 with DMUL + DFMA), but each lane reads 2 operand doubles per p instead of 12:
-// the kernel moves from the shared-memory roof (1184 clk per grid point and CTA) to the FP64-pipe roof (768 clk).
+// One grid point of the register-tile update.  `sl` = the grid point's slice inside the stage (block b of the stage at
+// sl + b * TP_BLK_BYTES).  hrq[a][b][c] accumulates H[p_a][r_c][q_b].
 template <bool DIAG>
-__device__ __forceinline__ void tp_update(const uint8_t* sl, const uint32_t (&offA)[8], const uint32_t (&offB)[8],
-                                          uint32_t offG, bool loads, double (&hq)[16][2], double (&hr)[16][2]) {
-  const double2 g = lds128(sl, offG);
-  double2 gt = make_double2(0.0, 0.0);
-  if (!DIAG) gt = lds128(sl, offG + (TP_OFF_GTQR0 - TP_OFF_GQR0));
+__device__ __forceinline__ void tp_update(const uint8_t* sl, const uint32_t (&offPQ)[4], const uint32_t (&offPR)[4],
+                                          const uint32_t (&offQR)[2], double (&hqr)[4][2][4], double (&hrq)[4][2][4]) {
+  double gqr[2][4], gt[2][4];            // gt[b][c] = G_I[r_c][q_b] (read from the transposed copy GT_I[q][r])
 #pragma unroll
-  for (int p = 0; p < 16; p++) {
-    double a = 0.0, b = 0.0;
-    if (loads) {                                    // lanes t = 0, 1 carry k = 0, 1; k = 2, 3 are zero
-      a = lds64(sl, offA[p & 7] + (p >> 3) * 1024);
-      b = lds64(sl, offB[p & 7] + (p >> 3) * 1024);
-    }
-    double s0 = 0.0, s1 = 0.0;
-    dmma884_tp(s0, s1, a, b);
-    hq[p][0] = fma(s0, g.x, hq[p][0]);
-    hq[p][1] = fma(s1, g.y, hq[p][1]);
+  for (int b = 0; b < 2; b++) {
+    double2 g0 = lds128(sl, offQR[b]), g1 = lds128(sl, (offQR[b] ^ 64));
+    gqr[b][0] = g0.x; gqr[b][1] = g0.y; gqr[b][2] = g1.x; gqr[b][3] = g1.y;
     if (!DIAG) {
-      hr[p][0] = fma(s0, gt.x, hr[p][0]);
-      hr[p][1] = fma(s1, gt.y, hr[p][1]);
+      double2 h0 = lds128(sl, 2 * TP_BLK_BYTES + offQR[b]), h1 = lds128(sl, 2 * TP_BLK_BYTES + (offQR[b] ^ 64));
+      gt[b][0] = h0.x; gt[b][1] = h0.y; gt[b][2] = h1.x; gt[b][3] = h1.y;
     }
+  }
+#pragma unroll
+  for (int a = 0; a < 4; a++) {
+    double2 e = lds128(sl, offPQ[a]), f = lds128(sl, TP_BLK_BYTES + offPQ[a]);
+    double2 e0 = lds128(sl, offPR[a]), e1 = lds128(sl, (offPR[a] ^ 64));
+    double2 f0 = lds128(sl, 2 * TP_BLK_BYTES + offPR[a]), f1 = lds128(sl, 2 * TP_BLK_BYTES + (offPR[a] ^ 64));
+    const double epq[2] = {e.x, e.y}, fpq[2] = {f.x, f.y};
+    const double epr[4] = {e0.x, e0.y, e1.x, e1.y}, fpr[4] = {f0.x, f0.y, f1.x, f1.y};
+#pragma unroll
+    for (int b = 0; b < 2; b++)
+#pragma unroll
+      for (int c = 0; c < 4; c++) {
+        const double sv = fma(epr[c], fpq[b], epq[b] * fpr[c]);
+        hqr[a][b][c] = fma(sv, gqr[b][c], hqr[a][b][c]);
+        if (!DIAG) hrq[a][b][c] = fma(sv, gt[b][c], hrq[a][b][c]);
+      }
   }
 }
 
-// E, F: tensor maps over [nI][nPp][NPp] (innermost NPp); G, GT: over [nI][NPp][NPp] with GT_I[q][r] = G_I[r][q] (the
-// mirrored block is read with the same row-q / column-r pattern as the direct one); box 16 x 16 x 1, SWIZZLE_128B.
+// E, F: tensor maps over [nI][nPp][NPp] (innermost NPp); G, GT: over [nI][NPp][NPp] with GT_I[q][r] = G_I[r][q] (so that the
+// mirrored block is read with the same row-q / chunk-r pattern as the direct one); box 16 x 16 x TP_IC, SWIZZLE_128B.
 // Grid points beyond nI (odd nI) are zero-filled by the TMA unit and add nothing.
 __global__ void __launch_bounds__(TP_THREADS, 1)
 triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_constant__ CUtensorMap mapF,
@@ -133,10 +122,14 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
   const uint32_t bar_full = ring + TP_STAGES * TP_STAGE_BYTES;
   const uint32_t bar_empty = bar_full + TP_STAGES * 8;
 
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, g = lane >> 2, t = lane & 3;
-  const int qb = warp >> 2, rb = warp & 3;              // this warp's 8 x 8 block of the 16 q x 32 r tile, all 16 p
-  const int pig = (g >> 1) + 4 * (g & 1);               // row g of the fragments <-> q = 8 qb + pi(g): rows g, g+1 differ in bit 2
-  const int qrow = 8 * qb + pig;                        // q inside the tile
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int wp = warp >> 2, wq = (warp >> 1) & 1, wr = warp & 1;
+  const int lp = lane >> 4, lq = ((lane >> 2) & 1) * 2 + ((lane >> 3) & 1), lr = lane & 3;   // lane bit 2 -> q bit 2
+  const int tp0 = wp * 8 + lp * 4;                      // 4 consecutive p
+  const int tq0 = wq * 8 + lq * 2;                      // 2 consecutive q
+  const int cq = tq0 >> 1;                              // 16-byte chunk of (.., tq0) in a 16-wide row
+  // r: this thread owns r = wr*16 + {2 lr, 2 lr + 1, 2 lr + 8, 2 lr + 9}  -> block wr, chunks lr and lr + 4
+
   const int my_items = p.n_items > (int)blockIdx.x ? (p.n_items - 1 - (int)blockIdx.x) / (int)gridDim.x + 1 : 0;
   const int nS = (p.nI + TP_IC - 1) / TP_IC;            // stages per work item
   const int total = my_items * nS;                      // < 2^31 (checked by the launcher)
@@ -145,34 +138,31 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
     for (int s = 0; s < TP_STAGES; s++) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, 8); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  __shared__ int prod[3];                               // producer counters (thread 0): flat fill index, item, stage in item
-  if (tid == 0) { prod[0] = 0; prod[1] = 0; prod[2] = 0; }
   __syncthreads();
 
+  // ---- producer (thread 0 only): flat fill index pj = (item pk of this CTA, stage pS of the item) ------------------------
+  // (its counters live in shared memory: the compute loop needs every register of the 255-register budget)
+  __shared__ int prod[3];
+  if (tid == 0) { prod[0] = 0; prod[1] = 0; prod[2] = 0; }
   auto fill = [&]() {
     int pj = prod[0], pk = prod[1], pS = prod[2];
     if (pj >= total) return;
     const TripleItem it = p.items[blockIdx.x + (long long)pk * gridDim.x];
-    const int s = pj % TP_STAGES, f = pj / TP_STAGES;
+    const int s = pj % TP_STAGES, f = pj / TP_STAGES, I = pS * TP_IC;
     if (f > 0) mbar_wait(bar_empty + 8 * s, (uint32_t)((f - 1) & 1));
-    const uint32_t bf = bar_full + 8 * s;
-    mbar_expect_tx(bf, TP_IC * (it.diag ? 8 : 10) * TP_BLK);
-#pragma unroll
-    for (int ii = 0; ii < TP_IC; ii++) {
-      const uint32_t dst = ring + s * TP_STAGE_BYTES + ii * TP_SLICE_BYTES;
-      const int I = pS * TP_IC + ii;
-      tma_load_3d(dst + TP_OFF_EPQ, &mapE, it.q0, it.p0, I, bf);
-      tma_load_3d(dst + TP_OFF_FPQ, &mapF, it.q0, it.p0, I, bf);
-      tma_load_3d(dst + TP_OFF_EPR0, &mapE, it.r0, it.p0, I, bf);
-      tma_load_3d(dst + TP_OFF_EPR1, &mapE, it.r0 + 16, it.p0, I, bf);
-      tma_load_3d(dst + TP_OFF_FPR0, &mapF, it.r0, it.p0, I, bf);
-      tma_load_3d(dst + TP_OFF_FPR1, &mapF, it.r0 + 16, it.p0, I, bf);
-      tma_load_3d(dst + TP_OFF_GQR0, &mapG, it.r0, it.q0, I, bf);
-      tma_load_3d(dst + TP_OFF_GQR1, &mapG, it.r0 + 16, it.q0, I, bf);
-      if (!it.diag) {
-        tma_load_3d(dst + TP_OFF_GTQR0, &mapGT, it.r0, it.q0, I, bf);
-        tma_load_3d(dst + TP_OFF_GTQR1, &mapGT, it.r0 + 16, it.q0, I, bf);
-      }
+    const uint32_t dst = ring + s * TP_STAGE_BYTES, bf = bar_full + 8 * s;
+    mbar_expect_tx(bf, it.diag ? 8 * TP_BLK_BYTES : 10 * TP_BLK_BYTES);
+    tma_load_3d(dst + 0 * TP_BLK_BYTES, &mapE, it.q0, it.p0, I, bf);
+    tma_load_3d(dst + 1 * TP_BLK_BYTES, &mapF, it.q0, it.p0, I, bf);
+    tma_load_3d(dst + 2 * TP_BLK_BYTES, &mapE, it.r0, it.p0, I, bf);
+    tma_load_3d(dst + 3 * TP_BLK_BYTES, &mapE, it.r0 + 16, it.p0, I, bf);
+    tma_load_3d(dst + 4 * TP_BLK_BYTES, &mapF, it.r0, it.p0, I, bf);
+    tma_load_3d(dst + 5 * TP_BLK_BYTES, &mapF, it.r0 + 16, it.p0, I, bf);
+    tma_load_3d(dst + 6 * TP_BLK_BYTES, &mapG, it.r0, it.q0, I, bf);
+    tma_load_3d(dst + 7 * TP_BLK_BYTES, &mapG, it.r0 + 16, it.q0, I, bf);
+    if (!it.diag) {
+      tma_load_3d(dst + 8 * TP_BLK_BYTES, &mapGT, it.r0, it.q0, I, bf);
+      tma_load_3d(dst + 9 * TP_BLK_BYTES, &mapGT, it.r0 + 16, it.q0, I, bf);
     }
     pj++;
     if (++pS == nS) { pS = 0; pk++; }
@@ -181,29 +171,31 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
   if (tid == 0)
     for (int n = 0; n < TP_LOOKAHEAD; n++) fill();
 
-  // ---- per-lane shared-memory byte offsets inside a grid point's slice (128-byte swizzle: chunk ^= address row & 7) ------
-  // A fragment (rows q): lanes t = 0 read E[p][q], t = 1 read F[p][q];  B fragment (columns r): t = 0 F[p][r], t = 1 E[p][r]
-  uint32_t offA[8], offB[8];
-  {
-    const int colA = qrow, colB = 8 * (rb & 1) + g;
-    const bool fA = (t == 1), fB = (t == 0);            // which of the two reads the F block
+  // ---- per-thread shared-memory byte offsets inside a grid point's slice (swizzle: chunk ^= row & 7) -------------------
+  uint32_t offPQ[4], offPR[4], offQR[2];
 #pragma unroll
-    for (int k = 0; k < 8; k++) {
-      offA[k] = (fA ? TP_OFF_FPQ : TP_OFF_EPQ) + k * 128 + ((((colA >> 1) ^ k ^ (fA ? 4 : 0)) << 4) | ((colA & 1) << 3));
-      offB[k] = (fB ? TP_OFF_FPR0 + (rb >> 1) * 3072 : TP_OFF_EPR0 + (rb >> 1) * 2048) + k * 128 +
-                ((((colB >> 1) ^ k ^ (fB ? 4 : 0)) << 4) | ((colB & 1) << 3));
-    }
+  for (int a = 0; a < 4; a++) {
+    const int row = tp0 + a;
+    offPQ[a] = row * 128 + ((cq ^ (row & 7)) << 4);
+    offPR[a] = (2 + wr) * TP_BLK_BYTES + row * 128 + ((lr ^ (row & 7)) << 4);        // chunk lr; chunk lr + 4 is ^ 64
   }
-  const uint32_t offG = TP_OFF_GQR0 + (rb >> 1) * 2048 + qrow * 128 + (((4 * (rb & 1) + t) ^ (qrow & 7)) << 4);
-  const bool loads = t < 2;
+#pragma unroll
+  for (int b = 0; b < 2; b++) {
+    const int row = tq0 + b;
+    offQR[b] = (6 + wr) * TP_BLK_BYTES + row * 128 + ((lr ^ (row & 7)) << 4);
+  }
 
-  double hq[16][2], hr[16][2];     // hq[p][e] -> H[p][q][r + e],  hr[p][e] -> H[p][r + e][q],  r = 8 rb + 2t
+  double hqr[4][2][4], hrq[4][2][4];
   int st = 0;                 // ring stage of the current iteration
   uint32_t par = 0;           // its mbarrier phase parity
   for (int k = 0; k < my_items; k++) {
     const int diag = p.items[blockIdx.x + (long long)k * gridDim.x].diag;
 #pragma unroll
-    for (int pp = 0; pp < 16; pp++) hq[pp][0] = hq[pp][1] = hr[pp][0] = hr[pp][1] = 0.0;
+    for (int a = 0; a < 4; a++)
+#pragma unroll
+      for (int b = 0; b < 2; b++)
+#pragma unroll
+        for (int c = 0; c < 4; c++) hqr[a][b][c] = hrq[a][b][c] = 0.0;
 
     for (int s = 0; s < nS; s++) {
       mbar_wait(bar_full + 8 * st, par);
@@ -212,10 +204,10 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
       const uint8_t* sl = ring_ptr + st * TP_STAGE_BYTES;
       if (diag) {
 #pragma unroll 1
-        for (int ii = 0; ii < TP_IC; ii++) tp_update<true>(sl + ii * TP_SLICE_BYTES, offA, offB, offG, loads, hq, hr);
+        for (int ii = 0; ii < TP_IC; ii++) tp_update<true>(sl + ii * TP_SLICE_BYTES, offPQ, offPR, offQR, hqr, hrq);
       } else {
 #pragma unroll 1
-        for (int ii = 0; ii < TP_IC; ii++) tp_update<false>(sl + ii * TP_SLICE_BYTES, offA, offB, offG, loads, hq, hr);
+        for (int ii = 0; ii < TP_IC; ii++) tp_update<false>(sl + ii * TP_SLICE_BYTES, offPQ, offPR, offQR, hqr, hrq);
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(bar_empty + 8 * st);
@@ -225,20 +217,28 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
     // ---- write back this item's block(s) of H[p][q][r] ---------------------------------------------------------------
     const TripleItem cur = p.items[blockIdx.x + (long long)k * gridDim.x];
     const long long sHp = (long long)p.NPp * p.NPp;
-    const int q = cur.q0 + qrow, r = cur.r0 + 8 * rb + 2 * t;
+    const int rA = cur.r0 + wr * 16 + 2 * lr;              // r = rA, rA + 1, rA + 8, rA + 9
 #pragma unroll
-    for (int pp = 0; pp < 16; pp++) {
-      double* Hp = p.H + (long long)(cur.p0 + pp) * sHp;
-      double2* d = reinterpret_cast<double2*>(Hp + (long long)q * p.NPp + r);
-      double2 v = make_double2(hq[pp][0], hq[pp][1]);
-      if (p.accumulate) { const double2 o = *d; v.x += o.x; v.y += o.y; }
-      *d = v;
+    for (int a = 0; a < 4; a++) {
+      double* Hp = p.H + (long long)(cur.p0 + tp0 + a) * sHp;
+#pragma unroll
+      for (int b = 0; b < 2; b++) {
+        double* row = Hp + (long long)(cur.q0 + tq0 + b) * p.NPp;
+        double2* d0 = reinterpret_cast<double2*>(row + rA);
+        double2* d1 = reinterpret_cast<double2*>(row + rA + 8);
+        double2 v0 = make_double2(hqr[a][b][0], hqr[a][b][1]), v1 = make_double2(hqr[a][b][2], hqr[a][b][3]);
+        if (p.accumulate) { double2 o0 = *d0, o1 = *d1; v0.x += o0.x; v0.y += o0.y; v1.x += o1.x; v1.y += o1.y; }
+        *d0 = v0; *d1 = v1;
+      }
       if (!cur.diag) {
-        double* m0 = Hp + (long long)r * p.NPp + q;
-        double* m1 = m0 + p.NPp;
-        double w0 = hr[pp][0], w1 = hr[pp][1];
-        if (p.accumulate) { w0 += *m0; w1 += *m1; }
-        *m0 = w0; *m1 = w1;
+#pragma unroll
+        for (int c = 0; c < 4; c++) {
+          const int r = rA + (c & 1) + 8 * (c >> 1);
+          double2* d = reinterpret_cast<double2*>(Hp + (long long)r * p.NPp + cur.q0 + tq0);
+          double2 vv = make_double2(hrq[a][0][c], hrq[a][1][c]);
+          if (p.accumulate) { double2 o = *d; vv.x += o.x; vv.y += o.y; }
+          *d = vv;
+        }
       }
     }
   }
