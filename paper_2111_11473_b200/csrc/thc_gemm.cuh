@@ -88,6 +88,21 @@ struct TileLoader {
   __device__ __forceinline__ void issue(double* s, const double* __restrict__ g, int kt, int K) const {
     const int k0 = kt * BK;
     const double* gk = g + (long long)kt * kstep;
+    if (k0 + BK <= K) {                                      // full k-tile (all but the last): no K-tail arithmetic
+#pragma unroll
+      for (int q = 0; q < NCH; q++) {
+        if (NCH * NTHREADS != CHUNKS && threadIdx.x + q * NTHREADS >= CHUNKS) continue;
+        const double* src = gk + goff[q];                    // rows beyond the operand point at row 0 and copy 0 bytes
+        double* dst = s + soff[q];
+        if (AL16) {
+          cp_async16(dst, src, bytes[q]);
+        } else {
+          cp_async8(dst, src, bytes[q] >= 8 ? 8 : 0);
+          cp_async8(dst + 1, bytes[q] >= 16 ? src + 1 : src, bytes[q] >= 16 ? 8 : 0);
+        }
+      }
+      return;
+    }
 #pragma unroll
     for (int q = 0; q < NCH; q++) {
       if (NCH * NTHREADS != CHUNKS && bytes[q] == 0 && threadIdx.x + q * NTHREADS >= CHUNKS) continue;
