@@ -29,6 +29,7 @@ struct GemmParams {
   int splits; long long sCs;      // split-K: partial tile stride (C then points at the partial buffer)
   double alpha, beta;
   double* Ct; long long ldct, sCtb;   // optional second output: Ct_b[n][m] = alpha * (A B^T)[m][n] (no aux, no beta)
+  int upper_only;                     // symmetric product: CTAs whose tile lies strictly below the diagonal do nothing
 };
 
 __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
@@ -138,6 +139,7 @@ __global__ void __launch_bounds__(WM* WN * 32) dgemm_kernel(const GemmParams p) 
   const int tile_m = blockIdx.x / tiles_n, tile_n = blockIdx.x % tiles_n;
   const int split = blockIdx.z % p.splits, b = blockIdx.z / p.splits;
   const int m0 = tile_m * BM, n0 = tile_n * BN;
+  if (p.upper_only && n0 + BN <= m0) return;       // whole tile has n < m: the caller mirrors it from the upper triangle
   const double* Ab = p.A + (long long)b * p.sAb;
   const double* Bb = p.B + (long long)b * p.sBb;
   const int ktiles = (p.K + BK - 1) / BK;
@@ -272,6 +274,7 @@ struct ReduceParams {
   int M, N, batch, splits;
   long long ldd, sDb, ldaux, sAuxb;
   double alpha, beta;
+  int skip_bm, skip_bn;     // upper-only product: elements of tiles (skip_bm x skip_bn) strictly below the diagonal are left alone
 };
 __global__ void reduce_splits_kernel(const ReduceParams p) {
   const long long per = (long long)p.batch * p.M * p.N;
@@ -280,6 +283,7 @@ __global__ void reduce_splits_kernel(const ReduceParams p) {
     long long r = idx / p.N;
     int m = (int)(r % p.M);
     int b = (int)(r / p.M);
+    if (p.skip_bm && (n / p.skip_bn + 1) * p.skip_bn <= (m / p.skip_bm) * p.skip_bm) continue;
     double s = 0.0;
     for (int sp = 0; sp < p.splits; sp++) s += p.part[(long long)sp * per + idx];
     s *= p.alpha;

@@ -77,6 +77,7 @@ struct Gemm {
   double alpha_ = 1.0, beta_ = 0.0;
   const double* aux_ = nullptr; i64 ldaux = 0, sAuxb = 0;
   double* ct_ = nullptr; i64 ldct = 0, sCtb = 0;
+  bool upper_ = false;
   // A(m,k): am == 'K' -> A[m*lda + k], 'M' -> A[k*lda + m].  B(n,k): bm == 'K' -> B[n*ldb + k], 'N' -> B[k*ldb + n].
   Gemm(const double* A_, i64 lda_, char am, const double* B_, i64 ldb_, char bm, double* C_, i64 ldc_, i64 M_, i64 N_, i64 K_)
       : M((int)M_), N((int)N_), K((int)K_), A(A_), lda(lda_), akm(am == 'K'), B(B_), ldb(ldb_), bkm(bm == 'K'), C(C_), ldc(ldc_) {}
@@ -85,6 +86,7 @@ struct Gemm {
   Gemm& ab(double a, double b) { alpha_ = a; beta_ = b; return *this; }
   Gemm& aux(const double* p, i64 ld, i64 sb) { aux_ = p; ldaux = ld; sAuxb = sb; return *this; }
   Gemm& transposed_copy(double* p, i64 ld, i64 sb) { ct_ = p; ldct = ld; sCtb = sb; return *this; }   // Ct_b[n][m] too
+  Gemm& upper_only() { upper_ = true; return *this; }    // symmetric M x M product: tiles strictly below the diagonal are skipped
 };
 
 // tile configurations of dgemm_kernel
@@ -175,7 +177,12 @@ struct Ctx {
     for (int cfg = 0; cfg < 3; cfg++) {
       const TileCfg& tc = TILE_CFGS[cfg];
       if (cfg < 2 && (g.M <= 64 || g.N <= (cfg == 0 ? 64 : 32))) continue;
-      const i64 tmn = (i64)((g.M + tc.BM - 1) / tc.BM) * ((g.N + tc.BN - 1) / tc.BN) * g.nbatch;
+      i64 tmn = (i64)((g.M + tc.BM - 1) / tc.BM) * ((g.N + tc.BN - 1) / tc.BN) * g.nbatch;
+      if (g.upper_) {                                       // only tiles that reach the diagonal or lie above it work
+        tmn = 0;
+        for (i64 tm = 0; tm * tc.BM < g.M; tm++)
+          for (i64 tn = 0; tn * tc.BN < g.N; tn++) tmn += ((tn + 1) * tc.BN > tm * tc.BM);
+      }
       const double slots = (double)h->sms * tc.per_sm;
       const int smax = g.ct_ ? 1 : (int)std::max<i64>(1, std::min<i64>(64, kiters / 8));   // the transposed copy is written by the main kernel only
       for (int sp = 1; sp <= smax; sp++) {
@@ -204,6 +211,7 @@ struct Ctx {
     p.kbatch = g.nkb; p.sAk = g.sAk; p.sBk = g.sBk;
     p.splits = splits; p.alpha = g.alpha_; p.beta = g.beta_;
     p.Ct = g.ct_; p.ldct = g.ldct; p.sCtb = g.sCtb;
+    p.upper_only = g.upper_ ? 1 : 0;
     if (splits > 1) { p.C = splitk; p.ldc = g.N; p.sCb = (i64)g.M * g.N; p.sCs = per; }
     else            { p.C = g.C; p.ldc = g.ldc; p.sCb = g.sCb; p.sCs = 0; }
 
@@ -218,7 +226,7 @@ struct Ctx {
     if (h->prof_mask & 1)
       snprintf(desc, sizeof desc, "gemm %s M=%d N=%d K=%d batch=%d kbatch=%d splits=%d %c%c%s", tile == 0 ? "big" : (tile == 1 ? "mid" : "small"), g.M, g.N, g.K,
                g.nbatch, g.nkb, splits, g.akm ? 'K' : 'M', g.bkm ? 'K' : 'N', al16 ? "" : " unaligned");
-    prof_start(0, desc, 2.0 * g.M * g.N * (double)g.K * g.nbatch * g.nkb);
+    prof_start(0, desc, 2.0 * g.M * g.N * (double)g.K * g.nbatch * g.nkb * (g.upper_ ? 0.5 * (1.0 + (double)tc.BN / g.N) : 1.0));
     const int sel = (g.akm ? 4 : 0) | (g.bkm ? 2 : 0) | (al16 ? 1 : 0);
     switch (sel) {
       case 7: e = launch_gemm_variant<true, true, true>(tile, grid, h->stream, p); break;
@@ -238,6 +246,7 @@ struct Ctx {
       r.M = g.M; r.N = g.N; r.batch = g.nbatch; r.splits = splits;
       r.ldd = g.ldc; r.sDb = g.sCb; r.ldaux = g.ldaux; r.sAuxb = g.sAuxb;
       r.alpha = g.alpha_; r.beta = g.beta_;
+      r.skip_bm = g.upper_ ? tc.BM : 0; r.skip_bn = g.upper_ ? tc.BN : 0;
       reduce_splits_kernel<<<ew_blocks(per), 256, 0, h->stream>>>(r);
       launched();
     }
@@ -300,6 +309,14 @@ struct Ctx {
     dim3 grid((unsigned)((n + 31) / 32), (unsigned)((n + 31) / 32)), blk(32, 8);
     prof_start(2, "symmetrize_kernel", 16.0 * n * n);
     symmetrize_kernel<<<grid, blk, 0, h->stream>>>(P, out, (int)n, scale);
+    launched();
+    prof_stop(2);
+  }
+  void mirror_upper(double* A, i64 n) {
+    if (dry || !ok()) return;
+    dim3 grid((unsigned)((n + 31) / 32), (unsigned)((n + 31) / 32)), blk(32, 8);
+    prof_start(2, "mirror_upper_kernel", 8.0 * n * n);
+    mirror_upper_kernel<<<grid, blk, 0, h->stream>>>(A, (int)n);
     launched();
     prof_stop(2);
   }

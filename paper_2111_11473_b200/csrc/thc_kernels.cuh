@@ -172,6 +172,22 @@ __global__ void symmetrize_kernel(const double* __restrict__ Pm, double* __restr
   }
 }
 
+// A[m][n] = A[n][m] for m > n   (completes a symmetric matrix whose GEMM computed the upper triangle only)
+__global__ void mirror_upper_kernel(double* __restrict__ A, int n) {
+  __shared__ double tile[32][33];
+  const int bx = blockIdx.x, by = blockIdx.y;          // source tile (rows by, cols bx) with by <= bx
+  if (by > bx) return;
+  for (int j = threadIdx.y; j < 32; j += blockDim.y) {
+    int r = by * 32 + j, c = bx * 32 + threadIdx.x;
+    if (r < n && c < n) tile[j][threadIdx.x] = A[(i64)r * n + c];
+  }
+  __syncthreads();
+  for (int j = threadIdx.y; j < 32; j += blockDim.y) {
+    int r = bx * 32 + j, c = by * 32 + threadIdx.x;    // destination element (r, c) = source (c, r)
+    if (r < n && c < n && r > c) A[(i64)r * n + c] = tile[threadIdx.x][j];
+  }
+}
+
 // FooT[i][j] = delta_ij eps[i] + xi_oo[j][i];  Fvv[a][b] = delta_ab eps[o+a] + xi_vv[a][b]   (Alg.9 lines 5-6 l.823-827)
 __global__ void fock_kernel(const double* __restrict__ eps, const double* __restrict__ xi_oo, const double* __restrict__ xi_vv,
                             double* __restrict__ FooT, double* __restrict__ Fvv, int o, int v) {

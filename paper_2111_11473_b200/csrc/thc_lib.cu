@@ -146,7 +146,8 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out, const Shard& sh
         // H4: D^l = C^l Z ;  s1 += sum_l D^l C^l^T                                                   (Alg.1 lines 14-15)
         double* D = Mv;   // Mv is dead after the combine
         c.gemm(Gemm(Mo, NP, 'K', in.Z, NP, 'K', D, NP, nl * NP, NP, NP));
-        c.gemm(Gemm(D, NP, 'K', Mo, NP, 'K', s1, NP, NP, NP, NP).kbatch(nl, NP2, NP2).ab(1.0, 1.0));
+        // (sigma1 = sum_l C^l Z C^l^T is symmetric: only the tiles on and above the diagonal are computed)
+        c.gemm(Gemm(D, NP, 'K', Mo, NP, 'K', s1, NP, NP, NP, NP).kbatch(nl, NP2, NP2).ab(1.0, 1.0).upper_only());
       }
       ar.release(m0);
     }
@@ -176,6 +177,8 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out, const Shard& sh
       ar.release(m0);
     }
   }
+
+  if (local && do_s1) c.mirror_upper(s1, NP);          // complete the symmetric sigma1 from its upper triangle
 
   // ---- H7: s2 = A A^T + Dm A^T + A Dm^T  (Alg.2 line 13 l.559; rows of Aa/Dm are Cholesky vectors) --------------------
   if (!local) {
