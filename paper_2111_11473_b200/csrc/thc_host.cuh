@@ -182,6 +182,7 @@ struct Ctx {
         tmn = 0;
         for (i64 tm = 0; tm * tc.BM < g.M; tm++)
           for (i64 tn = 0; tn * tc.BN < g.N; tn++) tmn += ((tn + 1) * tc.BN > tm * tc.BM);
+        tmn *= g.nbatch;
       }
       const double slots = (double)h->sms * tc.per_sm;
       const int smax = g.ct_ ? 1 : (int)std::max<i64>(1, std::min<i64>(64, kiters / 8));   // the transposed copy is written by the main kernel only
@@ -312,10 +313,10 @@ struct Ctx {
     launched();
     prof_stop(2);
   }
-  void mirror_upper(double* A, i64 n) {
+  void mirror_upper(double* A, i64 n, i64 nbatch = 1) {     // nbatch matrices n x n, densely packed
     if (dry || !ok()) return;
-    dim3 grid((unsigned)((n + 31) / 32), (unsigned)((n + 31) / 32)), blk(32, 8);
-    prof_start(2, "mirror_upper_kernel", 8.0 * n * n);
+    dim3 grid((unsigned)((n + 31) / 32), (unsigned)((n + 31) / 32), (unsigned)nbatch), blk(32, 8);
+    prof_start(2, "mirror_upper_kernel", 8.0 * n * n * nbatch);
     mirror_upper_kernel<<<grid, blk, 0, h->stream>>>(A, (int)n);
     launched();
     prof_stop(2);

@@ -175,6 +175,7 @@ __global__ void symmetrize_kernel(const double* __restrict__ Pm, double* __restr
 // A[m][n] = A[n][m] for m > n   (completes a symmetric matrix whose GEMM computed the upper triangle only)
 __global__ void mirror_upper_kernel(double* __restrict__ A, int n) {
   __shared__ double tile[32][33];
+  A += (i64)blockIdx.z * n * n;                        // grid.z = batch of densely packed n x n matrices
   const int bx = blockIdx.x, by = blockIdx.y;          // source tile (rows by, cols bx) with by <= bx
   if (by > bx) return;
   for (int j = threadIdx.y; j < 32; j += blockDim.y) {

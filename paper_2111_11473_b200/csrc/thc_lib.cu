@@ -135,11 +135,17 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out, const Shard& sh
       double *Mo = ar.alloc(nl * NP2), *Mv = ar.alloc(nl * NP2);
       // H1: T1T[P][(l,j)] = sum_i Xo[i,P] B^l_ij ;  Mo^l[P][Q] = sum_j T1T[P][(l,j)] Xo[j,Q]      (Alg.1 lines 6-7)
       c.gemm(Gemm(XoT, o, 'K', in.B_oo + L0 * o * o, o, 'K', T1T, nl * o, NP, nl * o, o));
-      c.gemm(Gemm(T1T, nl * o, 'K', XoT, o, 'K', Mo, NP, NP, NP, o).batch(nl, o, 0, NP2));
+      // (B^l symmetric => M^{o,l}, M^{v,l} symmetric: for NP of several tiles only the upper tiles are computed and the
+      //  lower ones mirrored in one batched pass; for small NP the mirror pass costs more than it saves)
+      const bool sym_half = NP >= 640;
+      Gemm gMo = Gemm(T1T, nl * o, 'K', XoT, o, 'K', Mo, NP, NP, NP, o).batch(nl, o, 0, NP2);
+      c.gemm(sym_half ? gMo.upper_only() : gMo);
       // H2: same with the vv block                                                                  (Alg.1 lines 10-11)
       c.gemm(Gemm(XvT, v, 'K', bvv, v, 'K', T2T, nl * v, NP, nl * v, v));
       if (streamed && !c.dry && h->bvv_mode == THC_BVV_HOST) c.bvv_release(blk);
-      c.gemm(Gemm(T2T, nl * v, 'K', XvT, v, 'K', Mv, NP, NP, NP, v).batch(nl, v, 0, NP2));
+      Gemm gMv = Gemm(T2T, nl * v, 'K', XvT, v, 'K', Mv, NP, NP, NP, v).batch(nl, v, 0, NP2);
+      c.gemm(sym_half ? gMv.upper_only() : gMv);
+      if (sym_half) { c.mirror_upper(Mo, NP, nl); c.mirror_upper(Mv, NP, nl); }
       // H3: C^l = v .* Mo^l - o .* Mv^l (in place over Mo);  C3 += Mo^l .* Mv^l                   (Alg.1 l.8,12,13; Alg.3 l.7)
       c.combine(Mo, Mv, omat, vmat, C3, NP2, nl);
       if (do_s1) {
