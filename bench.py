@@ -199,7 +199,7 @@ def run_ours(args):
     o, v, NL, NP, NX = c["o"], c["v"], c["NL"], c["NP"], c["NX"]
     # N = 1: the whole evaluation on one GPU.  N > 1: ONE evaluation sharded over the ranks as the paper shards it
     # (Cholesky ranges + row blocks of the T2^2 terms, one NCCL all-reduce) -> strong scaling.
-    sharded = world > 1
+    sharded = world > 1 or bool(os.environ.get("THC_BENCH_FORCE_SHARDED"))    # the env switch exercises the sharded code path on one rank
     L0, L1, _, _ = thc.thc_shard_range(NL, NP, rank, world)
     provider = args.config >= 4                      # B_vv (304 GB) is generated block by block on the device
     if args.config <= 2:
