@@ -20,6 +20,8 @@
  *       Xo[o][NP]  Xv[v][NP]  Z[NP][NP] (symmetric)  B_oo[NL][o][o]  B_ov[NL][o][v]  B_vv[NL][v][v] (each
  *       B^L symmetric)  Y[o+v][NX] (occupied rows first)  V[NX][NX] (symmetric)  eps[o+v] (occupied first)
  *       R[NP][NP].
+ *   - Z, V and every B^L are ASSUMED symmetric (not checked) and the library relies on it: symmetric products
+ *     (sigma1, the half-transforms M^{o,L}, M^{v,L}, the energy reduction) are evaluated on the upper triangle and mirrored.
  *   - "device pointer" = memory of the handle's CUDA device; "host pointer" = ordinary host memory (pinned
  *     memory makes the copies asynchronous but is not required).
  *   - The caller owns every input and output buffer; inputs are never modified.  The library owns only the
