@@ -13,10 +13,12 @@
 // B200 design
 //   * persistent CTAs (one per SM, 256 threads = 8 warps as 2p x 2q x 2r; lane = 2p x 4q x 4r; thread tile 4p x 2q x 4r
 //     plus its mirror = 64 FP64 accumulators), CTA tile 16p x 16q x 32r (+ mirror 16p x 32r x 16q);
-//   * operands are fetched by TMA (cp.async.bulk.tensor.3d, SWIZZLE_128B) as ten 16x16 FP64 blocks (2 KB each) per grid
-//     point I into a TP_STAGES-deep shared-memory ring; full/empty mbarriers, no __syncthreads in the I loop.  The TMA
-//     issue is done by lane 0 of warp (j mod 8) at iteration j, for iteration j + TP_STAGES - 2 (two iterations of slack
-//     on the empty barrier), so the ring keeps ~120 KB in flight per SM;
+//   * operands are fetched by TMA (cp.async.bulk.tensor.3d, SWIZZLE_128B) as ten boxes of 16 x 16 x TP_IC FP64 values
+//     (TP_IC = 2 grid points, 4 KB per box) into a TP_STAGES-deep shared-memory ring; full/empty mbarriers, no
+//     __syncthreads in the I loop.  Thread 0 issues the boxes of stage j + TP_STAGES - 2 when it enters stage j (two
+//     stages of slack on the empty barrier; its counters live in shared memory), so ~120 KB are in flight per SM.  The
+//     mirrored block is read from a transposed copy of G (written by the GEMM epilogue) so that it has the same
+//     row-q / column-r access pattern as the direct one;
 //   * the 128-byte swizzle makes every 16-byte fragment load bank-conflict free (rows 4 apart differ in chunk bit 2);
 //   * work items (p-tile, q-tile, r-tile) come from a host-built list ordered in groups of 8 p-tiles x 6 q-tiles x 3
 //     r-tiles, so that the ~148 CTAs running at the same time share their operand tiles in L2 (5x less HBM traffic).
