@@ -97,13 +97,14 @@ struct Gemm {
 #define THC_BIG 128, 128, THC_BIG_BK, 2, 4, THC_BIG_ST
 #define THC_MID 128, 64, 16, 4, 2, 4
 #define THC_SMALL 64, 64, 16, 2, 2, 4
+#define THC_TINYK 64, 64, 16, 2, 2, 2      // K <= 32: the whole K in the two stages, six CTAs per SM hide each other's latency
 constexpr int BIG_THREADS = 256, SMALL_THREADS = 128;
 constexpr int gemm_smem_bytes(int BM, int BN, int BK, int ST, bool akm, bool bkm) {
   return ST * ((akm ? BM * BK : BK * (BM + 2)) + (bkm ? BN * BK : BK * (BN + 2))) * 8;
 }
-// tile 0: 128x128 (one CTA per SM), 1: 128x64 (two), 2: 64x64 (three)
+// tile 0: 128x128 (one CTA per SM), 1: 128x64 (two), 2: 64x64 (three), 3: 64x64 with a 2-stage ring for K <= 32 (six)
 struct TileCfg { int BM, BN, per_sm; double lone_rate, pipe_share; };
-constexpr TileCfg TILE_CFGS[3] = {{128, 128, 1, 1.0, 1.0}, {128, 64, 2, 0.7, 0.9}, {64, 64, 3, 0.5, 0.75}};
+constexpr TileCfg TILE_CFGS[4] = {{128, 128, 1, 1.0, 1.0}, {128, 64, 2, 0.7, 0.9}, {64, 64, 3, 0.5, 0.75}, {64, 64, 6, 0.5, 0.75}};
 
 template <bool AKM, bool BKM, bool AL16>
 static cudaError_t launch_gemm_variant(int tile, dim3 grid, cudaStream_t st, const GemmParams& p) {
@@ -119,12 +120,16 @@ static cudaError_t launch_gemm_variant(int tile, dim3 grid, cudaStream_t st, con
     static bool done = false;
     if (!done) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, sm); done = true; }
     k<<<grid, BIG_THREADS, sm, st>>>(p);
-  } else {
+  } else if (tile == 2) {
     auto k = dgemm_kernel<THC_SMALL, AKM, BKM, AL16>;
     int sm = gemm_smem_bytes(64, 64, 16, 4, AKM, BKM);
     static bool done = false;
     if (!done) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, sm); done = true; }
     k<<<grid, SMALL_THREADS, sm, st>>>(p);
+  } else {
+    auto k = dgemm_kernel<THC_TINYK, AKM, BKM, AL16>;
+    int sm = gemm_smem_bytes(64, 64, 16, 2, AKM, BKM);
+    k<<<grid, SMALL_THREADS, sm, st>>>(p);         // 32 KB of shared memory: no opt-in needed
   }
   return cudaPeekAtLastError();
 }
@@ -197,6 +202,7 @@ struct Ctx {
         if (t < best * (sp > 1 ? 0.97 : 1.0)) { best = t; tile = cfg; splits = sp; }
       }
     }
+    if (tile == 2 && kiters <= 2 && splits == 1) tile = 3;      // tiny K: latency-bound CTAs, run six per SM
     const TileCfg& tc = TILE_CFGS[tile];
     const i64 tiles_mn = (i64)((g.M + tc.BM - 1) / tc.BM) * ((g.N + tc.BN - 1) / tc.BN);
     const i64 per = (i64)g.nbatch * g.M * g.N;
@@ -225,7 +231,7 @@ struct Ctx {
     cudaError_t e;
     char desc[160];
     if (h->prof_mask & 1)
-      snprintf(desc, sizeof desc, "gemm %s M=%d N=%d K=%d batch=%d kbatch=%d splits=%d %c%c%s", tile == 0 ? "big" : (tile == 1 ? "mid" : "small"), g.M, g.N, g.K,
+      snprintf(desc, sizeof desc, "gemm %s M=%d N=%d K=%d batch=%d kbatch=%d splits=%d %c%c%s", tile == 0 ? "big" : (tile == 1 ? "mid" : (tile == 2 ? "small" : "tinyK")), g.M, g.N, g.K,
                g.nbatch, g.nkb, splits, g.akm ? 'K' : 'M', g.bkm ? 'K' : 'N', al16 ? "" : " unaligned");
     prof_start(0, desc, 2.0 * g.M * g.N * (double)g.K * g.nbatch * g.nkb * (g.upper_ ? 0.5 * (1.0 + (double)tc.BN / g.N) : 1.0));
     const int sel = (g.akm ? 4 : 0) | (g.bkm ? 2 : 0) | (al16 ? 1 : 0);
