@@ -513,7 +513,7 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
                                   : std::max<int64_t>(1, ((int64_t)2 << 30) / (NX * NX * 8));
   h->bP7 = std::min<int64_t>(NP, (opt && opt->bP7) ? opt->bP7 : p7_auto);
   h->bX = std::min<int64_t>(pad_to(NP, 16), (opt && opt->bX) ? pad_to(opt->bX, 16) : pad_to(NP, 16));
-  h->bI = std::min<int64_t>(NX, (opt && opt->bI) ? opt->bI : 512);   // long I loops amortise the H read-modify-write
+  h->bI = std::min<int64_t>(NX, (opt && opt->bI) ? opt->bI : 1024);   // long I loops amortise the H read-modify-write
   int64_t cap = opt ? opt->workspace_bytes_max : 0;
   if (cap == 0) {
     DeviceGuard g(dev);
@@ -542,7 +542,7 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
       const double t_g = fNX * (2 * fo * fv * fNP + 2 * fo * fNP * fNP + 2 * fo * fv * fNX) / 25e12;       // DMMA, s
       const double t_h = 16.0 * fNP * (double)pad_to(NP, 32) * (double)pad_to(NP, 32) / 5e12;            // HBM, s
       double best = 1e300; int64_t bestX = 0, bestI = 0;
-      for (int64_t bi : {16, 24, 32, 48, 64, 96, 128, 192, 256, 384, 512}) {
+      for (int64_t bi : {16, 24, 32, 48, 64, 96, 128, 192, 256, 384, 512, 768, 1024}) {
         if (bi > NX) break;
         h->bI = bi; h->bX = 16;
         if (need_device(h) > cap) break;
