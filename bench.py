@@ -35,8 +35,9 @@ SMS, DFMA_LANES_PER_SM = 148, 64
 FALLBACK_BF16_TFLOPS, FALLBACK_HBM_GBS, FALLBACK_SM_MAX_MHZ = 1590.0, 6650.0, 1965.0
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed `ncu --set full`
-# capture (profiles/), keyed by (config, kernel class); None until captured.
-NCU_TRAFFIC_BYTES = {}
+# capture (profiles/), keyed by (config, kernel class); None until captured.  For a class of many launches (gemm) it is
+# the class's DRAM bytes of one evaluation / its launches per evaluation.  Source: profiles/r01_dram_traffic.md.
+NCU_TRAFFIC_BYTES = {(1, "gemm"): 93.26e6, (2, "triple"): 804.5e9}
 
 
 def measured_peaks():

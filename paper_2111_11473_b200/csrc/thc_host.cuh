@@ -448,7 +448,7 @@ struct Ctx {
     const cuuint32_t box[3] = {16, 16, (cuuint32_t)TP_IC}, es[3] = {1, 1, 1};
     CUresult r = reinterpret_cast<EncodeFn>(h->encode_tiled)(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, const_cast<double*>(base), dims,
                                                              strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
-                                                             CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                                                             CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) { check(cudaErrorInvalidValue); return false; }
     return true;
   }
