@@ -2,17 +2,23 @@
 """Benchmark of the THC-RR-CCSD projected doubles residual + energy on B200 (BASELINE.json metric).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+                    [--bvv device|host|provider] [--trace FILE] [--probe] [--no-cpu-baseline]
 
 One "step" = one pass of the whole hot path: thc_residual (R_PQ, all six terms)
-followed by thc_energy_device, on one seeded synthetic input set of BASELINE.json config C (default 1).
-Prints ONE JSON line (rank 0).  See DESIGN.md section 8 for how every field is measured.
+followed by thc_energy_device, on one seeded synthetic input set of BASELINE.json config C.  The default workload is
+config 3 (o=150, v=850, NL=3000, NP=2500, NX=5000), the largest configuration whose 25 evaluations fit the driver's
+bench window; config 4 takes ~13 minutes per evaluation and is benched with --config 4.
+Prints ONE JSON line (rank 0).  DESIGN.md section 8 says how every field is measured.
 
---impl reference times the CPU oracle (oracle/dense.py) as it stands on the host cores; this and the
-`cpu_baseline` leg are the only places that execute anything under oracle/.
+--impl reference times the CPU oracle (oracle/) as it stands on the host cores; this and the `cpu_baseline` leg are
+the only places that execute anything under oracle/.  --probe prints the measured FP64 / shared-memory ceilings of
+the device (the denominators DESIGN.md section 7 discusses) instead of running the benchmark.
 """
 import argparse
+import csv
 import json
 import os
+import socket
 import statistics
 import subprocess
 import sys
@@ -29,15 +35,13 @@ INPUT_NAMES = ("Xo", "Xv", "Z", "B_ov", "B_oo", "B_vv", "Y", "V", "eps")
 # Nominal figures used for the FP64 roofline denominators:
 #   FP64 tensor (DMMA): MEASURED_PEAKS.json bf16_tflops x (nominal FP64 tensor 45 / nominal bf16 2250), the ratio
 #   of /opt/skills/guides/blackwell_cuda_programming.md's table;  FP64 FMA pipe: 148 SMs x 64 DFMA lanes x 2 flop
-#   x SM clock.
+#   x SM clock.  The same-run yardsticks (`extra.yardstick`) show what the pipe really delivers.
 NOMINAL_FP64_TENSOR_OVER_BF16 = 45.0 / 2250.0
 SMS, DFMA_LANES_PER_SM = 148, 64
 FALLBACK_BF16_TFLOPS, FALLBACK_HBM_GBS, FALLBACK_SM_MAX_MHZ = 1590.0, 6650.0, 1965.0
-
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed `ncu --set full`
-# capture (profiles/), keyed by (config, kernel class); None until captured.  For a class of many launches (gemm) it is
-# the class's DRAM bytes of one evaluation / its launches per evaluation.  Source: profiles/r01_dram_traffic.md.
-NCU_TRAFFIC_BYTES = {(1, "gemm"): 93.26e6, (2, "triple"): 804.5e9}
+# DRAM bytes per launch of a kernel class from a committed `ncu --set full` capture: profiles/<this file>, one row per
+# (config, class) with the command that produced it.  No row -> roofline.traffic is null.
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_dram_traffic.csv")
 
 
 def measured_peaks():
@@ -50,89 +54,115 @@ def measured_peaks():
                 sm_max_mhz=FALLBACK_SM_MAX_MHZ, source="fallback")
 
 
+def ncu_traffic(config, cls):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu summary, or None."""
+    if not os.path.exists(TRAFFIC_CSV):
+        return None
+    with open(TRAFFIC_CSV) as f:
+        for row in csv.DictReader(f):
+            if int(row["config"]) == config and row["class"] == cls:
+                return float(row["dram_bytes_per_launch"])
+    return None
+
+
+# ======================================================================================================================
+# CPU oracle legs (cpu_baseline and --impl reference)
+# ======================================================================================================================
 def dense_oracle_flops(o, v, NL):
     """Rough flop count of the dense oracle: ERI builds + the Omega contractions."""
     return 2.0 * (o ** 2 * v ** 4 + o ** 4 * v ** 2 + 6 * o ** 3 * v ** 3) + 2.0 * NL * v ** 4
 
 
-def time_oracle(cfg, reps, budget_s=30.0):
-    """Time oracle/dense.py on config `cfg` if its dense arrays fit (configs 0, 1); for larger configs time
-    config 1 and scale by the dense-oracle flop ratio (stated in `sample`)."""
-    import numpy as np
-    from thc_synth import make_config, config_dims
-    from oracle import dense
-    run_cfg = cfg if cfg <= 1 else 1
-    x = make_config(run_cfg)
-    times = []
-    t_all = time.perf_counter()
-    for _ in range(max(1, reps)):
+class OracleSample:
+    """A bounded sample of one oracle evaluation of config `cfg`, and the factor that scales its time to a whole one.
+
+    configs 0, 1: the dense oracle (oracle/dense.py), the whole evaluation (scale 1).
+    configs 2-4 : the dense arrays do not fit host memory, so the oracle of record there is the sampled-row oracle
+                  (oracle/rows.py).  The sample is one row R[P, :] of all six terms over the FIRST `nl` Cholesky vectors
+                  (+ the xi intermediates and the energy over the same vectors); a whole evaluation is NP rows, and the
+                  Cholesky-dependent work (sigma1, sigma2, sigma3, xi, E) grows by NL / nl.  Both factors are stated in
+                  `sample`.
+    """
+
+    def __init__(self, cfg, nl=None):
+        from thc_synth import CONFIGS, make_inputs
+        c = CONFIGS[cfg]
+        self.cfg, self.c = cfg, c
+        if cfg <= 1:
+            self.x = make_inputs(c["o"], c["v"], c["NL"], c["NP"], c["NX"], c["seed"])
+            self.kind = "dense"
+            self.sample = f"one full dense-oracle evaluation of config {cfg}"
+        else:
+            self.nl = nl or {2: 8, 3: 2, 4: 1}[cfg]
+            self.x = make_inputs(c["o"], c["v"], c["NL"], c["NP"], c["NX"], c["seed"], l_keep=self.nl)
+            self.kind = "rows"
+            self.P = c["NP"] // 2
+            self.sample = (f"sampled-row oracle (oracle/rows.py) on config {cfg}: one row P={self.P} of sigma1..sigma9, xi and E "
+                           f"over the first {self.nl} of {c['NL']} Cholesky vectors; a whole evaluation = NP={c['NP']} rows, "
+                           f"Cholesky-dependent parts x{c['NL'] / self.nl:.0f}")
+
+    def run(self):
+        """Returns the estimated seconds of ONE whole oracle evaluation of the config."""
+        import numpy as np
+        x = self.x
+        if self.kind == "dense":
+            from oracle import dense
+            t0 = time.perf_counter()
+            res = dense.residual_and_energy(x.Xo, x.Xv, x.Z, x.B_ov, x.B_oo, x.B_vv, x.Y, x.V, x.eps)
+            dt = time.perf_counter() - t0
+            assert np.isfinite(res["R"]).all()
+            return dt
+        from oracle.rows import RowOracle
+        ro = RowOracle(x.Xo, x.Xv, x.Z, x.B_ov, x.B_oo, x.B_vv, x.Y, x.V, x.eps, lblock=self.nl)
+        c, lscale = self.c, self.c["NL"] / self.nl
         t0 = time.perf_counter()
-        res = dense.residual_and_energy(x.Xo, x.Xv, x.Z, x.B_ov, x.B_oo, x.B_vv, x.Y, x.V, x.eps)
-        times.append(time.perf_counter() - t0)
-        assert np.isfinite(res["R"]).all()
-        if time.perf_counter() - t_all > budget_s:
-            break
-    t = statistics.median(times)
+        ro.xi(); ro.energy()
+        t_once = (time.perf_counter() - t0) * lscale                       # once per evaluation, all L
+        t0 = time.perf_counter()
+        r = ro.row(self.P, terms=("s1", "s2", "s3"))
+        t_lin = (time.perf_counter() - t0) * lscale                        # per row, all L
+        t0 = time.perf_counter()
+        r.update(ro.row(self.P, terms=("s6", "s7", "s9")))
+        t_quad = time.perf_counter() - t0                                  # per row, no L dependence
+        assert all(np.isfinite(v).all() for v in r.values())
+        return t_once + c["NP"] * (t_lin + t_quad)
+
+
+def time_oracle(cfg, budget_s=30.0):
     cores = len(os.sched_getaffinity(0))
-    if run_cfg == cfg:
-        value, sample = 1.0 / t, f"{len(times)} full dense-oracle evaluation(s) of config {cfg} (median)"
-    else:
-        o, v, NL, _, _ = config_dims(cfg)
-        o1, v1, NL1, _, _ = config_dims(1)
-        scale = dense_oracle_flops(o, v, NL) / dense_oracle_flops(o1, v1, NL1)
-        value = 1.0 / (t * scale)
-        sample = (f"{len(times)} full dense-oracle evaluation(s) of config 1, extrapolated to config {cfg} by the "
-                  f"dense-oracle flop ratio {scale:.3g} (its dense t/ERI arrays do not fit host memory at config {cfg})")
-    return dict(value=value, unit=UNIT, cores=cores, kind="oracle", sample=sample, seconds_per_eval=1.0 / value)
+    s = OracleSample(cfg)
+    times, t_all = [], time.perf_counter()
+    while len(times) < 3 and (not times or time.perf_counter() - t_all < budget_s):
+        times.append(s.run())
+    t = statistics.median(times)
+    return dict(value=1.0 / t, unit=UNIT, cores=cores, kind="oracle", sample=f"{s.sample}; median of {len(times)} run(s)",
+                seconds_per_eval=t)
 
 
 def run_reference(args):
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
+    if int(os.environ.get("RANK", "0")) != 0:
         return
     from thc_synth import config_dims
     o, v, NL, NP, NX = config_dims(args.config)
-    n = args.steps + args.warmup
-    per_eval_budget = 150.0 / max(1, n)
-    import numpy as np
-    from thc_synth import make_config
-    from oracle import dense
-    run_cfg = args.config if args.config <= 1 else 1
-    x = make_config(run_cfg)
-
-    def step():
-        res = dense.residual_and_energy(x.Xo, x.Xv, x.Z, x.B_ov, x.B_oo, x.B_vv, x.Y, x.V, x.eps)
-        assert np.isfinite(res["R"]).all()
-
-    # each step is one full dense-oracle evaluation unless that would take the run past a few minutes; then a
-    # step is the oracle on config 0 scaled by the flop ratio (bounded sample)
-    t0 = time.perf_counter(); step(); first = time.perf_counter() - t0
-    sample_cfg = run_cfg
-    if first > per_eval_budget and run_cfg != 0:
-        sample_cfg = 0
-        x = make_config(0)
-    for _ in range(max(0, args.warmup - 1)):
-        step()
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
-        step()
-    dt = (time.perf_counter() - t0) / args.steps
-    so, sv, sNL, _, _ = config_dims(sample_cfg)
-    scale = dense_oracle_flops(o, v, NL) / dense_oracle_flops(so, sv, sNL)
-    value = 1.0 / (dt * scale)
+    s = OracleSample(args.config)
+    for _ in range(args.warmup):
+        s.run()
+    times = [s.run() for _ in range(args.steps)]
+    dt = sum(times) / len(times)
     cores = len(os.sched_getaffinity(0))
-    sample = (f"each step = one full dense-oracle evaluation of config {sample_cfg}" +
-              ("" if sample_cfg == args.config else f", extrapolated to config {args.config} by flop ratio {scale:.3g}"))
+    value = 1.0 / dt
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": dt * scale * 1e3, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"config{args.config}", "o": o, "v": v, "NL": NL, "NP": NP, "NX": NX},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": f"each step = {s.sample}"},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
 
 
+# ======================================================================================================================
 class ClockSampler:
     """nvidia-smi clocks/throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
@@ -145,7 +175,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.idx), f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
         except OSError:
             self.proc = None
@@ -178,6 +208,53 @@ class ClockSampler:
                 "reasons": sorted(reasons)}
 
 
+def yardstick(thc, torch, dev, n=8192):
+    """FP64 GEMM n^3 through the library's own DMMA kernel (thc_dgemm) and through torch.matmul (cuBLAS), best of 3
+    after one warm-up, TFLOP/s each: what the FP64 tensor pipe delivers in this very run.  cuBLAS is
+    a yardstick only, never on the product path."""
+    out = {}
+    try:
+        g = torch.Generator(device=dev).manual_seed(7)
+        A = torch.randn(n, n, dtype=torch.float64, device=dev, generator=g)
+        B = torch.randn(n, n, dtype=torch.float64, device=dev, generator=g)
+        C = torch.empty(n, n, dtype=torch.float64, device=dev)
+        hy = thc.thc_setup(4, 8, 4, 16, 16)
+
+        def best(fn):
+            fn()
+            ts = []
+            for _ in range(3):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(); fn(); b.record(); b.synchronize()
+                ts.append(a.elapsed_time(b))
+            return 2.0 * n ** 3 / (min(ts) * 1e-3) / 1e12
+        out["thc_dgemm_8192_tflops"] = best(lambda: hy.thc_dgemm(1, 1, n, n, n, 1.0, A, n, B, n, 0.0, C, n))
+        out["torch_matmul_fp64_8192_tflops"] = best(lambda: torch.matmul(A, B.T, out=C))
+        hy.close()
+        del A, B, C
+        torch.cuda.empty_cache()
+    except Exception as exc:          # the yardstick must never take the benchmark down (e.g. memory at config 4)
+        out["error"] = repr(exc)
+    return out
+
+
+def respawn_under_torchrun(args):
+    """`python bench.py --gpus N` (N > 1) without a launcher: start N ranks, one per GPU, through torch.distributed.run.
+    Fails loudly when the node has fewer GPUs -- never a silent N = 1 run."""
+    import torch
+    have = torch.cuda.device_count()
+    if have < args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} requested but this node has {have} CUDA device(s)")
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")            # the communicator lines show the ranks / NVLS in the log
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd, env=env))
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -188,11 +265,16 @@ def run_ours(args):
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}")
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the THC residual has no CPU path)")
+    if torch.cuda.device_count() <= local_rank:
+        raise SystemExit(f"bench.py: rank {rank} has no GPU (LOCAL_RANK {local_rank}, {torch.cuda.device_count()} visible)")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     if world > 1:
+        os.environ.setdefault("NCCL_DEBUG", "INFO")
         dist.init_process_group("nccl", device_id=dev)
     thc.lib()      # fails loudly if the extension is missing
 
@@ -200,9 +282,9 @@ def run_ours(args):
     o, v, NL, NP, NX = c["o"], c["v"], c["NL"], c["NP"], c["NX"]
     # N = 1: the whole evaluation on one GPU.  N > 1: ONE evaluation sharded over the ranks as the paper shards it
     # (Cholesky ranges + row blocks of the T2^2 terms, one NCCL all-reduce) -> strong scaling.
-    sharded = world > 1 or bool(os.environ.get("THC_BENCH_FORCE_SHARDED"))    # the env switch exercises the sharded code path on one rank
+    sharded = world > 1
     L0, L1, _, _ = thc.thc_shard_range(NL, NP, rank, world)
-    provider = args.config >= 4                      # B_vv (304 GB) is generated block by block on the device
+    bvv_mode = args.bvv or ("provider" if args.config >= 4 else "device")
     if args.config <= 2:
         x = make_inputs(o, v, NL, NP, NX, seed=c["seed"])
         host = [torch.from_numpy(np.ascontiguousarray(getattr(x, n))).pin_memory() for n in INPUT_NAMES]
@@ -215,25 +297,32 @@ def run_ours(args):
         dd = synth.make_inputs_device(o, v, NL, NP, NX, c["seed"], device=dev, with_bvv=False)
         if sharded:
             dd["B_ov"], dd["B_oo"] = dd["B_ov"][L0:L1].contiguous(), dd["B_oo"][L0:L1].contiguous()
-        if not provider:
+        if bvv_mode != "provider":
             dd["B_vv"] = synth.bvv_block(c["seed"], o, v, NL, L0, L1, dev)
         d = [dd[nm] for nm in INPUT_NAMES]
         host = [None if t is None else t.cpu().pin_memory() for t in d]
-    if provider:
+        del dd
+    if bvv_mode == "provider":
         from thc_synth import device as synth
 
         def bvv_fill(Lg, nl, dst):                   # thc_bvv_provider: fills B_vv[Lg:Lg+nl] on the library's stream
             synth.bvv_block(c["seed"], o, v, NL, Lg, Lg + nl, dev, out=dst)
         d[5] = bvv_fill
         host[5] = bvv_fill
+    elif bvv_mode == "host":                         # B_vv stays in pinned host memory and is streamed per L-block
+        d[5] = host[5]
+    torch.cuda.synchronize()
+    torch.cuda.empty_cache()
     R = torch.empty(NP, NP, dtype=torch.float64, device=dev)
     E = torch.zeros(1, dtype=torch.float64, device=dev)
     R_host = torch.empty(NP, NP, dtype=torch.float64).pin_memory()
-    h = thc.thc_setup(o, v, NL, NP, NX, bvv_mode="provider" if provider else "device")
+    yard = yardstick(thc, torch, dev) if rank == 0 else {}
+    h = thc.thc_setup(o, v, NL, NP, NX, bvv_mode=bvv_mode)
     flops = h.algorithmic_flops
+    alg_work = h.algorithmic_work
     input_bytes = sum(t.numel() * 8 for t in host if torch.is_tensor(t))
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
     use_flush = input_bytes < (512 << 20)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if use_flush else None     # > 126 MB L2
     if sharded:
         from paper_2111_11473_b200.sharded import CudaBackend, residual_sharded, energy_sharded
         backend = CudaBackend(h, *d)
@@ -252,18 +341,23 @@ def run_ours(args):
             dist.barrier()
             torch.cuda.synchronize()
 
-    # ---- warm-up (also finds the dominant kernel class) ----
+    # ---- warm-up (the last warm-up step is profiled per kernel class and finds the dominant class) ----
     W = max(3, args.warmup)
     for _ in range(W - 1):
         step()
     h.thc_profile_begin(7)
     step()
     prof_w = h.thc_profile_end()
-    work_w = h.thc_profile_work()        # executed flop (gemm, triple) / algorithmic HBM bytes (ew) of that step
+    work_w = h.thc_profile_work()        # EXECUTED flop (gemm, triple) / algorithmic HBM bytes (ew) of that step
+    if args.trace and rank == 0:
+        with open(args.trace, "w") as f:
+            f.write("class,ms,work,rate_T_per_s,description\n")
+            for cls, ms, work, desc in h.thc_profile_launches():
+                f.write(f"{cls},{ms:.4f},{work:.6g},{work / max(ms, 1e-9) / 1e9:.3f},\"{desc}\"\n")
     dominant = max(prof_w, key=lambda k: prof_w[k][0])
     dom_bit = {"gemm": 1, "triple": 2, "ew": 4}[dominant]
 
-    # ---- timed region: K steps, device-timed, L2 flushed between steps ----
+    # ---- timed region: K steps, device-timed per step, L2 flushed between steps when the inputs fit L2 ----
     sampler = ClockSampler(local_rank)
     sampler.start()
     time.sleep(0.3)
@@ -291,117 +385,152 @@ def run_ours(args):
     total_s = float(total_ms.item()) * 1e-3
     value = (1 if sharded else world) * K / total_s
     E_val = float(E.item())
+    blocks = h.blocks
 
     # ---- end to end through thc_residual_host: pinned host buffers in, R + E back on the host, every step ----
-    # (N > 1: the sharded evaluation has no host-buffer entry; its inputs are copied H2D explicitly every step)
-    def e2e_step():
-        if sharded:
-            dh = [t.to(dev, non_blocking=True) if torch.is_tensor(t) else t for t in host]
-            be = CudaBackend(h, *dh)
-            R_host.copy_(residual_sharded(be), non_blocking=True)
-            Eh = energy_sharded(be).cpu()
-            torch.cuda.synchronize()
-            return float(Eh[0])
-        return h.thc_residual_host(*host, R_host)       # synchronous
+    # The device-resident copies of the inputs are released first: the host entry stages its own copies inside the
+    # workspace, so its handle is set up with a cap that leaves room for them (same memory budget as above).
+    # Same L2 treatment as the device-timed leg (flush before each step when the inputs fit L2, outside the timer).
+    # (N > 1: the sharded evaluation has no host-buffer entry; its inputs are copied H2D explicitly every step.)
+    e2e_value, Ke = None, 0
+    if True:
+        if not sharded:
+            h.close()
+            del d
+            torch.cuda.empty_cache()
+            free_b, _ = torch.cuda.mem_get_info(dev)
+            cap = int(0.92 * free_b) - input_bytes - NP * NP * 8 - (64 << 20)
+            he = thc.thc_setup(o, v, NL, NP, NX, bvv_mode=bvv_mode, workspace_bytes_max=max(cap, 1 << 28))
 
-    Ke = max(1, min(K, 5 if args.config == 2 else (1 if args.config >= 3 else K)))
-    if args.config >= 4:
-        # config 4: staging copies of the 38 GB of resident inputs do not fit beside them and the workspace
-        Ke, e2e_value = 0, None
-    else:
-        e2e_step()
+        def e2e_step():
+            if sharded:
+                dh = [t.to(dev, non_blocking=True) if torch.is_tensor(t) else t for t in host]
+                be = CudaBackend(h, *dh)
+                R_host.copy_(residual_sharded(be), non_blocking=True)
+                Eh = energy_sharded(be).cpu()
+                torch.cuda.synchronize()
+                return float(Eh[0])
+            return he.thc_residual_host(*host, R_host)       # synchronous
+
+        Ke = max(1, min(K, 5 if args.config == 2 else (1 if args.config >= 3 else K)))
+        if args.config <= 2:
+            e2e_step()                                        # warm-up of the host entry (workspace allocation)
         barrier()
-        t0 = time.perf_counter()
-        for _ in range(Ke):
+        e2e_t = 0.0
+        for k in range(Ke):
+            if use_flush:
+                flush.fill_(k & 0xFF)
+                torch.cuda.synchronize()
+            t0 = time.perf_counter()
             e2e_step()
+            e2e_t += time.perf_counter() - t0
         barrier()
-        e2e_s = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
+        e2e_s = torch.tensor([e2e_t], dtype=torch.float64, device=dev)
         if world > 1:
             dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
         e2e_value = (1 if sharded else world) * Ke / float(e2e_s.item())
+        if not sharded:
+            he.close()
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel class ----
+    # ---- rooflines: ALGORITHMIC work / measured class time; executed work as a separate ratio ----
     pk = measured_peaks()
+    tensor_peak = pk["bf16"] * NOMINAL_FP64_TENSOR_OVER_BF16
+    alu_peak = SMS * DFMA_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
+    spec = {"gemm": ("tensor", "TFLOP/s", tensor_peak, 1e12,
+                     f"{pk['source']} bf16 burst {pk['bf16']:.1f} TFLOP/s x nominal FP64-tensor/bf16 ratio 45/2250"),
+            "triple": ("alu", "TFLOP/s", alu_peak, 1e12,
+                       f"148 SMs x 64 FP64 FMA lanes x 2 flop x {pk['sm_max_mhz']:.0f} MHz (max SM clock, {pk['source']})"),
+            "ew": ("hbm", "GB/s", pk["hbm"], 1e9, f"{pk['source']} copy bandwidth")}
+    names = {"gemm": "dgemm kernels (FP64 DMMA, all GEMM chains)", "triple": "triple_product_kernel (Alg.6 line 11)",
+             "ew": "Hadamard / reduction kernels"}
+
+    def class_roof(cls, ms, launches_n, executed):
+        bound, unit, peak, scale, src = spec[cls]
+        # ew: the class's work is HBM bytes (every operand element once per launch), identical executed / algorithmic
+        alg = executed if cls == "ew" else alg_work[cls]
+        ach = alg / (ms * 1e-3) / scale if ms > 0 else None
+        r = {"bound": bound, "kernel": names[cls], "achieved": ach, "peak": peak, "unit": unit, "peak_source": src,
+             "frac": ach / peak if ach else None, "ms": ms, "launches": launches_n,
+             "algorithmic_work": alg, "executed_over_algorithmic": executed / alg if alg else None}
+        return r
+
     dom_ms, dom_n = prof[dominant]
-    per_eval_ms = dom_ms / K
-    fo, fv, fNL, fNP, fNX = float(o), float(v), float(NL), float(NP), float(NX)
-    triple_flops = 5.0 * fNX * fNP ** 3
-    ew_flops = 5.0 * fNL * fNP * fNP
-    if dominant == "triple":
-        alg = triple_flops
-        peak = SMS * DFMA_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
-        roof = {"bound": "alu", "kernel": "triple_product_kernel (Alg.6 line 11)", "achieved": alg / (per_eval_ms * 1e-3) / 1e12,
-                "peak": peak, "unit": "TFLOP/s",
-                "peak_source": f"148 SMs x 64 FP64 FMA lanes x 2 flop x {pk['sm_max_mhz']:.0f} MHz (max SM clock, {pk['source']})"}
-    elif dominant == "gemm":
-        alg = flops - triple_flops - ew_flops
-        peak = pk["bf16"] * NOMINAL_FP64_TENSOR_OVER_BF16
-        roof = {"bound": "tensor", "kernel": "dgemm_kernel (FP64 DMMA, all GEMM chains)", "achieved": alg / (per_eval_ms * 1e-3) / 1e12,
-                "peak": peak, "unit": "TFLOP/s",
-                "peak_source": f"{pk['source']} bf16 {pk['bf16']:.1f} TFLOP/s x nominal FP64-tensor/bf16 ratio 45/2250"}
-    else:
-        alg = 0.0
-        roof = {"bound": "hbm", "kernel": "Hadamard/reduction kernels", "achieved": None, "peak": pk["hbm"], "unit": "GB/s",
-                "peak_source": f"{pk['source']} copy bandwidth"}
-    if roof["achieved"] is not None:
-        roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["traffic"] = NCU_TRAFFIC_BYTES.get((args.config, dominant))
-    roof["launches_per_step"] = dom_n / K
-    roof["ms_per_step"] = per_eval_ms
-    roof["share_of_step"] = per_eval_ms / (1e3 * total_s / K)
+    roof = class_roof(dominant, dom_ms / K, dom_n / K, work_w[dominant])
+    roof["traffic"] = ncu_traffic(args.config, dominant)
+    roof["launches_per_step"] = roof.pop("launches")
+    roof["ms_per_step"] = roof.pop("ms")
+    roof["share_of_step"] = roof["ms_per_step"] / (1e3 * total_s / K)
     roof["class_ms_warmup_step"] = {k: round(prof_w[k][0], 4) for k in prof_w}
-    # every kernel class of one profiled warm-up step against its own roof (EXECUTED work, recomputation included)
-    dmma_probe = SMS * DFMA_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
-    per_class = {}
-    for k, (unit, peak, bound) in {"gemm": ("TFLOP/s", pk["bf16"] * NOMINAL_FP64_TENSOR_OVER_BF16, "tensor"),
-                                   "triple": ("TFLOP/s", dmma_probe, "alu"),
-                                   "ew": ("GB/s", pk["hbm"], "hbm")}.items():
-        ms_k = prof_w[k][0]
-        if ms_k <= 0:
-            continue
-        ach = work_w[k] / (ms_k * 1e-3) / (1e12 if unit == "TFLOP/s" else 1e9)
-        per_class[k] = {"bound": bound, "achieved": ach, "peak": peak, "unit": unit, "frac": ach / peak,
-                        "ms": round(ms_k, 4), "launches": prof_w[k][1]}
-    per_class["gemm"]["frac_of_dmma_issue_rate"] = per_class["gemm"]["achieved"] / dmma_probe if "gemm" in per_class else None
+    per_class = {k: class_roof(k, prof_w[k][0], prof_w[k][1], work_w[k]) for k in prof_w if prof_w[k][0] > 0}
+    for k in per_class:
+        per_class[k].pop("kernel"); per_class[k].pop("peak_source")
+        per_class[k]["share_of_step"] = per_class[k]["ms"] / sum(prof_w[j][0] for j in prof_w)
+    if "gemm" in per_class:
+        per_class["gemm"]["frac_of_sustained_peak"] = per_class["gemm"]["achieved"] / (pk["bf16_sustained"] * NOMINAL_FP64_TENSOR_OVER_BF16)
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": 1e3 * total_s / K, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"config{args.config}", "o": o, "v": v, "NL": NL, "NP": NP, "NX": NX, "seed": c["seed"],
-                       "blocks": h.blocks, "l2": "flushed between steps (256 MiB write)" if use_flush else "inputs larger than L2",
+                       "blocks": blocks, "l2": "flushed between steps (256 MiB write), both legs" if use_flush else "inputs larger than L2",
                        "parallelism": "1 GPU" if world == 1 else f"one evaluation sharded over {world} GPUs (Cholesky ranges + T2^2 row blocks, one all-reduce)",
-                       "B_vv": "provider callback, generated per L-block on the device" if provider else "resident in HBM"},
+                       "B_vv": {"provider": "provider callback, generated per L-block on the device",
+                                "host": "pinned host memory, streamed per L-block", "device": "resident in HBM"}[bvv_mode]},
             "tflops_fp64_algorithmic": (1 if sharded else world) * flops * K / total_s / 1e12,
             "algorithmic_flops_per_eval": flops, "energy_Eh": E_val,
             "wall_s_timed_region": wall, "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": input_bytes, "d2h_bytes_per_step": NP * NP * 8 + 8,
                     "steps": Ke},
-            "gpu_launches": launches, "roofline": roof, "rooflines_by_class": per_class}
+            "gpu_launches": launches, "roofline": roof, "rooflines_by_class": per_class,
+            "extra": {"yardstick": yard}}
     if world == 1 and not args.no_cpu_baseline:
-        line["cpu_baseline"] = time_oracle(args.config, reps=3)
+        line["cpu_baseline"] = time_oracle(args.config)
     print(json.dumps(line), flush=True)
-    h.close()
+    if sharded:
+        h.close()
     if world > 1:
         dist.destroy_process_group()
+
+
+def run_probe(args):
+    """Measured ceilings of this device for the FP64 kernels (thc_probe in the library): DMMA and DFMA issue rates,
+    both interleaved, shared-memory -> register bandwidth by access width."""
+    import torch
+    import paper_2111_11473_b200 as thc
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --probe: no CUDA device")
+    h = thc.thc_setup(4, 8, 4, 16, 16)
+    out = {"probe": h.thc_probe(), "device": torch.cuda.get_device_name(0)}
+    out["yardstick"] = yardstick(thc, torch, torch.device("cuda", 0))
+    h.close()
+    print(json.dumps(out), flush=True)
 
 
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4])
+    ap.add_argument("--config", type=int, default=3, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--bvv", default=None, choices=["device", "host", "provider"],
+                    help="where B_vv lives (default: device; provider at config 4)")
+    ap.add_argument("--trace", default=None, help="write the per-launch records of the profiled warm-up step to this CSV")
+    ap.add_argument("--probe", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.probe:
+        run_probe(args)
     else:
+        if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+            respawn_under_torchrun(args)
         run_ours(args)
 
 

@@ -20,8 +20,9 @@
  *       Xo[o][NP]  Xv[v][NP]  Z[NP][NP] (symmetric)  B_oo[NL][o][o]  B_ov[NL][o][v]  B_vv[NL][v][v] (each
  *       B^L symmetric)  Y[o+v][NX] (occupied rows first)  V[NX][NX] (symmetric)  eps[o+v] (occupied first)
  *       R[NP][NP].
- *   - Z, V and every B^L are ASSUMED symmetric (not checked) and the library relies on it: symmetric products
- *     (sigma1, the half-transforms M^{o,L}, M^{v,L}, the energy reduction) are evaluated on the upper triangle and mirrored.
+ *   - Z, V and every B^L are ASSUMED symmetric and the library relies on it: symmetric products (sigma1, the
+ *     half-transforms M^{o,L}, M^{v,L}, the energy reduction) are evaluated on the upper triangle and mirrored.  The
+ *     hot path does not check; thc_options.check_symmetry turns on a debug pass that does.
  *   - "device pointer" = memory of the handle's CUDA device; "host pointer" = ordinary host memory (pinned
  *     memory makes the copies asynchronous but is not required).
  *   - The caller owns every input and output buffer; inputs are never modified.  The library owns only the
@@ -30,7 +31,7 @@
  *   - Device entry points enqueue work on the handle's stream (thc_set_stream; default stream 0) and return
  *     without synchronising; outputs are valid after the stream has been synchronised.
  *   - Every function returns THC_OK (0) or a negative thc_status; nothing throws or aborts.  The failing CUDA
- *     error (if any) is kept in the handle: thc_last_cuda_error.
+ *     error (if any) is kept in the handle: thc_last_error.
  *   - Pointers must be 8-byte aligned; 16-byte alignment (and even o, v, NP, NX) selects the vectorised
  *     load path, anything else the scalar one.  There is no CPU fallback of any kind.
  */
@@ -51,7 +52,7 @@ typedef enum {
   THC_ERR_INVALID_ARG = -1,   /* null pointer, non-positive size, misaligned pointer            */
   THC_ERR_OVERFLOW = -2,      /* a buffer size does not fit in 63 bits                          */
   THC_ERR_NO_MEMORY = -3,     /* workspace too small / cudaMalloc failed                        */
-  THC_ERR_CUDA = -4,          /* a CUDA call or kernel launch failed (see thc_last_cuda_error)  */
+  THC_ERR_CUDA = -4,          /* a CUDA call or kernel launch failed (see thc_last_error)       */
   THC_ERR_NO_DEVICE = -5,     /* no sm_100 device visible                                       */
   THC_ERR_PROVIDER = -6       /* a thc_bvv_provider callback returned non-zero                   */
 } thc_status;
@@ -79,10 +80,20 @@ typedef struct {
   int64_t bP7;              /* amplitude-grid rows per block of Alg.7 (0 = auto)                            */
   int64_t bX;               /* amplitude-grid rows per block of Alg.6 (0 = auto; rounded up to 16)          */
   int64_t bI;               /* ERI-grid points per chunk of Alg.6 (0 = auto)                                */
-  int64_t workspace_bytes_max; /* cap for the auto block-size choice (0 = 75 % of free device memory)       */
+  int64_t workspace_bytes_max; /* cap for the auto block-size choice (0 = 92 % of free device memory)       */
+  int64_t tma_min_flop;     /* GEMMs of at least this many flop with 16-byte aligned K-major operands run on the   */
+                            /* TMA-fed persistent kernel, smaller ones on the cp.async kernel (0 = default 2e8,     */
+                            /* -1 = never; tests use 1 to exercise the TMA kernel on small ragged shapes)           */
   int32_t term_mask;        /* THC_TERM_* bits, 0 = all                                                     */
   int32_t device;           /* CUDA device ordinal, -1 = current device                                     */
   int32_t bvv_mode;         /* thc_bvv_mode: what the B_vv argument of thc_residual[_terms] is                  */
+  int32_t check_symmetry;   /* debug: non-zero = every residual call first verifies, in one extra pass over HBM  */
+                            /* and one host synchronisation, that Z, V, every B^L_oo and (resident B_vv only)    */
+                            /* every B^L_vv are symmetric to 1e-12 of their largest element; an unsymmetric      */
+                            /* input makes the call return THC_ERR_INVALID_ARG instead of a silently wrong R     */
+  int32_t use_graph;        /* 1 = capture the evaluation into a CUDA graph on first use and replay it while the */
+                            /* pointers stay the same (launch-bound small shapes); 0 = never; -1 = auto: on when */
+                            /* the shape is launch-bound (< 2e10 algorithmic flop) and B_vv is resident          */
   int32_t reserved;         /* must be 0                                                                    */
 } thc_options;
 
@@ -105,16 +116,21 @@ int thc_set_stream(thc_handle* h, void* cuda_stream);
 int thc_get_blocks(const thc_handle* h, int64_t out[4]);
 
 /* R_PQ (device pointers; asynchronous).  Argument order follows the north_star:
- * thc_residual(X^o, X^v, Z, B_ov, B_oo, B_vv, Y, V, eps) -> R_PQ.                                     */
+ * thc_residual(X^o, X^v, Z, B_ov, B_oo, B_vv, Y, V, eps) -> R_PQ.
+ * B_vv is typed const void* because its meaning depends on thc_options.bvv_mode: THC_BVV_DEVICE a device pointer
+ * (const double*) to B_vv[NL][v][v]; THC_BVV_HOST a host pointer (const double*) to the same array; THC_BVV_PROVIDER
+ * a const thc_bvv_provider*.  The same holds for thc_residual_terms and thc_residual_shard (there: the rank's own
+ * slice, or, for a provider, the global L index is passed to fill); thc_residual_host takes a host array in the first
+ * two modes and a provider in the third.                                                               */
 int thc_residual(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
-                 const double* B_oo, const double* B_vv, const double* Y, const double* V, const double* eps,
+                 const double* B_oo, const void* B_vv, const double* Y, const double* V, const double* eps,
                  double* R);
 
 /* As thc_residual, and also writes each term separately (device pointers, any of them may be NULL):
  * terms[0..5] = sigma1, sigma2, sigma3, sigma6, sigma7, sigma9, each [NP][NP];  xi_oo[o][o] (Eq.39 l.280),
  * xi_vv[v][v] (Eq.40 l.283).  R may be NULL.                                                            */
 int thc_residual_terms(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
-                       const double* B_oo, const double* B_vv, const double* Y, const double* V,
+                       const double* B_oo, const void* B_vv, const double* Y, const double* V,
                        const double* eps, double* R, double* const terms[6], double* xi_oo, double* xi_vv);
 
 /* Correlation energy E = sum_L [ 2 a^L.Z.a^L - sum_PQ Z_PQ E^L_PQ E^L_QP ] (factorised form of
@@ -141,7 +157,7 @@ int thc_energy_device(thc_handle* h, const double* Xo, const double* Xv, const d
 int thc_shard_range(int64_t NL, int64_t NP, int rank, int nranks, int64_t out[4]);
 int64_t thc_shard_doubles(const thc_handle* h);
 int thc_residual_shard(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
-                       const double* B_oo, const double* B_vv, const double* Y, const double* V, const double* eps,
+                       const double* B_oo, const void* B_vv, const double* Y, const double* V, const double* eps,
                        int rank, int nranks, double* packed);
 int thc_residual_finish(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* Y,
                         const double* V, const double* eps, double* packed, double* R, double* const terms[6]);
@@ -152,7 +168,7 @@ int thc_energy_shard(thc_handle* h, const double* Xo, const double* Xv, const do
  * R (and E if E_host != NULL), copies R device->host into R_host[NP][NP], synchronises.  The staging
  * buffers are part of the workspace (thc_workspace_bytes_host includes them).                       */
 int thc_residual_host(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
-                      const double* B_oo, const double* B_vv, const double* Y, const double* V,
+                      const double* B_oo, const void* B_vv, const double* Y, const double* V,
                       const double* eps, double* R_host, double* E_host);
 
 /* Number of kernels this handle has launched since creation (its own kernels only; no library calls). */
@@ -171,6 +187,18 @@ int thc_profile_end(thc_handle* h, double ms[3], int64_t counts[3]);
  * launched, recomputation included; 5 flop per (P,Q,R,I) of line 11 over the padded extents), algorithmic HBM bytes
  * (each operand element read once, each result written once) for class 2. */
 int thc_profile_work(const thc_handle* h, double work[3]);
+/* Per-launch records of the last thc_profile_end, in launch order: thc_profile_launches returns how many there are;
+ * thc_profile_launch copies record k: its class (0, 1, 2 as above), its device time in milliseconds, its work (as in
+ * thc_profile_work) and a NUL-terminated description (kernel, shape, tile) truncated to desc_bytes.  Any out pointer
+ * may be NULL. */
+int64_t thc_profile_launches(const thc_handle* h);
+int thc_profile_launch(const thc_handle* h, int64_t k, int* cls, double* ms, double* work, char* desc,
+                       int64_t desc_bytes);
+/* ALGORITHMIC work of one residual evaluation per kernel class (SURVEY.md 8(a) formulas; no symmetry savings, no
+ * recomputation, no padding): work[0] = flop of every GEMM-shaped step (H0-H2, H4-H10 without line 11), work[1] =
+ * 5 NX NP^3 flop of Alg.6 line 11, work[2] = 5 NL NP^2 flop of the H3 Hadamard combine.  Their sum is
+ * thc_algorithmic_flops. */
+int thc_algorithmic_work(const thc_handle* h, double work[3]);
 
 /* Bare FP64 DMMA GEMM of the library (the kernel every GEMM chain uses), exposed for tests and roofline
  * measurement:  C[M][N] = alpha * sum_k A(m,k) B(n,k) + beta * C,  A(m,k) = A[m*lda+k] if a_kmajor else
@@ -186,8 +214,17 @@ int thc_dgemm(thc_handle* h, int a_kmajor, int b_kmajor, int64_t M, int64_t N, i
 int thc_triple_product(thc_handle* h, int64_t nI, int64_t nPp, int64_t NPp, const double* E, const double* F,
                        const double* G, const double* GT, double* H, int accumulate);
 
+/* Measured FP64 / shared-memory ceilings of the handle's device (synchronous; ~0.3 s).  MEASURED_PEAKS.json has no
+ * FP64 entry, so the rooflines of DESIGN.md section 7 rest on these:  out[0] issue rate of the FP64 tensor instruction
+ * (mma.sync.m8n8k4.f64 = SASS DMMA.8x8x4) in TFLOP/s, out[1] DFMA issue rate in TFLOP/s, out[2] both interleaved 1:1 in
+ * one warp (sum of both, TFLOP/s; ~ out[0] means one shared pipe), out[3], out[4], out[5] shared memory -> register
+ * bandwidth with 4-, 8- and 16-byte conflict-free loads in bytes per clock per SM at the maximum SM clock, out[6] that
+ * clock in MHz, out[7] = 0. */
+int thc_probe(thc_handle* h, double out[8]);
+
 const char* thc_strerror(int status);
-int thc_last_cuda_error(const thc_handle* h);   /* the cudaError_t of the last THC_ERR_CUDA, else 0 */
+int thc_last_error(const thc_handle* h);        /* the cudaError_t of the last THC_ERR_CUDA on this handle, else 0 */
+int thc_last_cuda_error(const thc_handle* h);   /* older name of thc_last_error (same value)                       */
 
 #ifdef __cplusplus
 }

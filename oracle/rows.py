@@ -81,6 +81,32 @@ class RowOracle:
             self._xi = (xi_oo, xi_vv)
         return self._xi
 
+    def xi_oo_column(self, j):
+        """xi_oo[:, j] alone (Eq.39 l.280 with the index j fixed): for shapes where the full xi costs hours of CPU.
+        n[L,d] = sum_me (2 t_jm^de - t_jm^ed) B^L_me,  xi_oo[k,j] = sum_Ld B^L_kd n[L,d]."""
+        xo = self.Xo[j]
+        col = np.zeros(self.o)
+        lim = ("optimal", 2 ** 34)
+        for L0, L1 in self._lblocks():
+            B = self.B_ov[L0:L1]
+            n = 2.0 * np.einsum("P,dP,PQ,mQ,eQ,Lme->Ld", xo, self.Xv, self.Z, self.Xo, self.Xv, B, optimize=lim) \
+                - np.einsum("P,eP,PQ,mQ,dQ,Lme->Ld", xo, self.Xv, self.Z, self.Xo, self.Xv, B, optimize=lim)
+            col += np.einsum("Lkd,Ld->k", B, n, optimize=True)
+        return col
+
+    def xi_vv_row(self, b):
+        """xi_vv[b, :] alone (Eq.40 l.283 with the index b fixed):
+        n[L,m] = sum_le (2 t_ml^be - t_ml^eb) B^L_le,  xi_vv[b,c] = -sum_Lm n[L,m] B^L_mc."""
+        xv = self.Xv[b]
+        row = np.zeros(self.v)
+        lim = ("optimal", 2 ** 34)
+        for L0, L1 in self._lblocks():
+            B = self.B_ov[L0:L1]
+            n = 2.0 * np.einsum("mP,P,PQ,lQ,eQ,Lle->Lm", self.Xo, xv, self.Z, self.Xo, self.Xv, B, optimize=lim) \
+                - np.einsum("mP,eP,PQ,lQ,Q,Lle->Lm", self.Xo, self.Xv, self.Z, self.Xo, xv, B, optimize=lim)
+            row -= np.einsum("Lm,Lmc->c", n, B, optimize=True)
+        return row
+
     # ---- one row -----------------------------------------------------------------------------------------------------
     def row(self, P, terms=TERMS):
         """{term: R[P, :]} for the requested terms (each the projection of that term's Omega alone)."""

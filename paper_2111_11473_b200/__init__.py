@@ -22,8 +22,9 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
 SYMBOLS = ("thc_setup", "thc_destroy", "thc_workspace_bytes", "thc_workspace_bytes_host", "thc_set_workspace",
            "thc_set_stream", "thc_get_blocks", "thc_residual", "thc_residual_terms", "thc_energy",
            "thc_energy_device", "thc_residual_host", "thc_profile_begin", "thc_profile_end", "thc_profile_work", "thc_kernel_launches", "thc_algorithmic_flops", "thc_dgemm",
-           "thc_triple_product", "thc_strerror", "thc_last_cuda_error", "thc_shard_range", "thc_shard_doubles",
-           "thc_residual_shard", "thc_residual_finish", "thc_energy_shard")
+           "thc_triple_product", "thc_strerror", "thc_last_cuda_error", "thc_last_error", "thc_shard_range",
+           "thc_shard_doubles", "thc_residual_shard", "thc_residual_finish", "thc_energy_shard",
+           "thc_profile_launches", "thc_profile_launch", "thc_algorithmic_work", "thc_probe")
 
 TERM_NAMES = ("s1", "s2", "s3", "s6", "s7", "s9")
 TERM_BITS = dict(s1=1, s2=2, s3=4, s6=8, s7=16, s9=32)
@@ -52,8 +53,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 class _Options(ctypes.Structure):
     _fields_ = [("bL", ctypes.c_int64), ("bP7", ctypes.c_int64), ("bX", ctypes.c_int64), ("bI", ctypes.c_int64),
-                ("workspace_bytes_max", ctypes.c_int64), ("term_mask", ctypes.c_int32), ("device", ctypes.c_int32),
-                ("bvv_mode", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+                ("workspace_bytes_max", ctypes.c_int64), ("tma_min_flop", ctypes.c_int64), ("term_mask", ctypes.c_int32), ("device", ctypes.c_int32),
+                ("bvv_mode", ctypes.c_int32), ("check_symmetry", ctypes.c_int32), ("use_graph", ctypes.c_int32),
+                ("reserved", ctypes.c_int32)]
 
 
 BVV_MODES = dict(device=0, host=1, provider=2)
@@ -101,6 +103,13 @@ def lib() -> ctypes.CDLL:
     L.thc_profile_begin.argtypes = [VP, ctypes.c_int]
     L.thc_profile_end.argtypes = [VP, ctypes.POINTER(D * 3), ctypes.POINTER(I64 * 3)]
     L.thc_profile_work.argtypes = [VP, ctypes.POINTER(D * 3)]
+    L.thc_profile_launches.argtypes = [VP]
+    L.thc_profile_launches.restype = I64
+    L.thc_profile_launch.argtypes = [VP, I64, ctypes.POINTER(ctypes.c_int), ctypes.POINTER(D), ctypes.POINTER(D),
+                                     ctypes.c_char_p, I64]
+    L.thc_algorithmic_work.argtypes = [VP, ctypes.POINTER(D * 3)]
+    L.thc_last_error.argtypes = [VP]
+    L.thc_probe.argtypes = [VP, ctypes.POINTER(D * 8)]
     L.thc_residual_host.argtypes = [VP] + [P] * 10 + [ctypes.POINTER(D)]
     L.thc_kernel_launches.argtypes = [VP]
     L.thc_kernel_launches.restype = I64
@@ -127,7 +136,7 @@ def _check(st: int, h=None):
     if st != 0:
         msg = lib().thc_strerror(st).decode()
         if h is not None and st == -4:
-            msg += f" [cudaError {lib().thc_last_cuda_error(h)}]"
+            msg += f" [cudaError {lib().thc_last_error(h)}]"
         raise ThcError(f"thc status {st}: {msg}")
 
 
@@ -153,14 +162,15 @@ class Thc:
     """One problem shape (thc_setup ... thc_destroy).  Methods mirror the C entry points."""
 
     def __init__(self, o, v, NL, NP, NX, *, bL=0, bP7=0, bX=0, bI=0, workspace_bytes_max=0, term_mask=0,
-                 device=-1, torch_workspace=True, bvv_mode="device"):
+                 device=-1, torch_workspace=True, bvv_mode="device", check_symmetry=False, use_graph=-1, tma_min_flop=0):
         import torch
         if not torch.cuda.is_available():
             raise ThcError("no CUDA device: the THC residual has no CPU path")
         self.o, self.v, self.NL, self.NP, self.NX = o, v, NL, NP, NX
         self._h = ctypes.c_void_p()
         self.bvv_mode = bvv_mode
-        opt = _Options(bL, bP7, bX, bI, workspace_bytes_max, term_mask, device, BVV_MODES[bvv_mode], 0)
+        opt = _Options(bL, bP7, bX, bI, workspace_bytes_max, tma_min_flop, term_mask, device, BVV_MODES[bvv_mode],
+                       int(bool(check_symmetry)), int(use_graph), 0)
         _check(lib().thc_setup(ctypes.byref(self._h), o, v, NL, NP, NX, ctypes.byref(opt)))
         self._ws = None
         self._torch_ws = torch_workspace
@@ -298,7 +308,16 @@ class Thc:
         L0, L1, _, _ = thc_shard_range(self.NL, NP, rank, nranks)
         nl = L1 - L0
         packed = out if out is not None else torch.empty(self.shard_doubles, dtype=torch.float64, device=self._device)
-        bvv = self._slice_ptr(B_vv, "B_vv", nl * v * v) if self.bvv_mode == "device" else self._bvv_ptr(B_vv, _dev_ptr)
+        if self.bvv_mode == "device":
+            bvv = self._slice_ptr(B_vv, "B_vv", nl * v * v)
+        elif self.bvv_mode == "host":
+            # the C entry expects the rank's own slice (vector L_begin first); the whole host array is accepted too
+            import torch
+            if isinstance(B_vv, torch.Tensor) and B_vv.numel() == self.NL * v * v and nl != self.NL:
+                B_vv = B_vv.reshape(self.NL, v, v)[L0:L1]
+            bvv = ctypes.c_void_p(None) if nl == 0 else _host_ptr(B_vv, "B_vv", nl * v * v)
+        else:
+            bvv = self._bvv_ptr(B_vv, _dev_ptr)      # provider: fill() receives global Cholesky indices
         _check(lib().thc_residual_shard(
             self._h, _dev_ptr(Xo, "Xo", o * NP), _dev_ptr(Xv, "Xv", v * NP), _dev_ptr(Z, "Z", NP * NP),
             self._slice_ptr(B_ov, "B_ov", nl * o * v), self._slice_ptr(B_oo, "B_oo", nl * o * o), bvv,
@@ -349,6 +368,33 @@ class Thc:
         w = (ctypes.c_double * 3)()
         _check(lib().thc_profile_work(self._h, ctypes.byref(w)), self._h)
         return {k: w[i] for i, k in enumerate(("gemm", "triple", "ew"))}
+
+    def thc_profile_launches(self):
+        """[(class name, milliseconds, work, description)] of every launch timed by the last thc_profile_end."""
+        n = int(lib().thc_profile_launches(self._h))
+        out, names = [], ("gemm", "triple", "ew")
+        buf = ctypes.create_string_buffer(192)
+        for k in range(n):
+            cls, ms, work = ctypes.c_int(), ctypes.c_double(), ctypes.c_double()
+            _check(lib().thc_profile_launch(self._h, k, ctypes.byref(cls), ctypes.byref(ms), ctypes.byref(work), buf,
+                                            len(buf)), self._h)
+            out.append((names[cls.value], ms.value, work.value, buf.value.decode()))
+        return out
+
+    @property
+    def algorithmic_work(self):
+        """{class: algorithmic flop of one evaluation}: gemm (every GEMM-shaped step), triple (Alg.6 line 11), ew (H3)."""
+        w = (ctypes.c_double * 3)()
+        _check(lib().thc_algorithmic_work(self._h, ctypes.byref(w)), self._h)
+        return {k: w[i] for i, k in enumerate(("gemm", "triple", "ew"))}
+
+    def thc_probe(self):
+        """Measured ceilings of the device (thc.h): FP64 tensor / FMA issue rates, shared-memory load bandwidth."""
+        out = (ctypes.c_double * 8)()
+        _check(lib().thc_probe(self._h, ctypes.byref(out)), self._h)
+        return dict(dmma_tflops=out[0], dfma_tflops=out[1], dmma_plus_dfma_interleaved_tflops=out[2],
+                    lds32_bytes_per_clk_per_sm=out[3], lds64_bytes_per_clk_per_sm=out[4],
+                    lds128_bytes_per_clk_per_sm=out[5], sm_clock_mhz=out[6])
 
     def thc_residual_host(self, Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps, R_host, want_energy=True):
         """End-to-end entry: HOST tensors in, R written into the host tensor R_host, returns E (or None)."""

@@ -225,38 +225,53 @@ __global__ void __launch_bounds__(WM* WN * 32) dgemm_kernel(const GemmParams p) 
   }
   cp_async_wait<0>();
 
-  // epilogue
+  // epilogue.  The operands of a row of fragments (aux values, old C values for beta != 0) are loaded for all NT
+  // fragments first and only then combined and stored, so that their latencies overlap (one dependent load per stored
+  // fragment made the small-K products with an aux operand epilogue-bound).
   const bool partial = p.splits > 1;
   double* Cb = p.C + (long long)b * p.sCb + (partial ? (long long)split * p.sCs : 0);
-  const double* auxb = p.aux ? p.aux + (long long)b * p.sAuxb : nullptr;
+  const double* auxb = (p.aux && !partial) ? p.aux + (long long)b * p.sAuxb : nullptr;
+  const bool use_beta = !partial && p.beta != 0.0;
   const bool vec = ((p.ldc & 1) == 0) && ((reinterpret_cast<uintptr_t>(Cb) & 15) == 0);
+  const bool vec_aux = auxb && ((p.ldaux & 1) == 0) && ((reinterpret_cast<uintptr_t>(auxb) & 15) == 0);
+  const double alpha = partial ? 1.0 : p.alpha;
 #pragma unroll
   for (int i = 0; i < MT; i++) {
-    int m = m0 + wm * WTM + i * 8 + g;
+    const int m = m0 + wm * WTM + i * 8 + g;
     if (m >= p.M) continue;
+    double ax[NT][2], cx[NT][2];
 #pragma unroll
     for (int j = 0; j < NT; j++) {
-      int n = n0 + wn * WTN + j * 8 + 2 * t;
+      const int n = n0 + wn * WTN + j * 8 + 2 * t;
+      ax[j][0] = ax[j][1] = 1.0;
+      cx[j][0] = cx[j][1] = 0.0;
       if (n >= p.N) continue;
-      double v0 = acc[i][j][0], v1 = acc[i][j][1];
-      bool two = (n + 1 < p.N);
-      if (!partial) {
-        v0 *= p.alpha; v1 *= p.alpha;
-        if (auxb) {
-          v0 *= auxb[(long long)m * p.ldaux + n];
-          if (two) v1 *= auxb[(long long)m * p.ldaux + n + 1];
-        }
+      const bool two = (n + 1 < p.N);
+      if (auxb) {
+        const double* a = auxb + (long long)m * p.ldaux + n;
+        if (two && vec_aux) { const double2 v = *reinterpret_cast<const double2*>(a); ax[j][0] = v.x; ax[j][1] = v.y; }
+        else { ax[j][0] = a[0]; if (two) ax[j][1] = a[1]; }
       }
-      if (p.Ct != nullptr && !partial) {          // transposed copy, before aux / beta are applied to the main output
+      if (use_beta) {
+        const double* c = Cb + (long long)m * p.ldc + n;
+        if (two && vec) { const double2 v = *reinterpret_cast<const double2*>(c); cx[j][0] = v.x; cx[j][1] = v.y; }
+        else { cx[j][0] = c[0]; if (two) cx[j][1] = c[1]; }
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < NT; j++) {
+      const int n = n0 + wn * WTN + j * 8 + 2 * t;
+      if (n >= p.N) continue;
+      const bool two = (n + 1 < p.N);
+      const double r0 = acc[i][j][0] * alpha, r1 = acc[i][j][1] * alpha;
+      if (p.Ct != nullptr && !partial) {          // transposed copy: the bare product, before aux / beta
         double* ct = p.Ct + (long long)b * p.sCtb + (long long)n * p.ldct + m;
-        ct[0] = acc[i][j][0] * p.alpha;
-        if (two) ct[p.ldct] = acc[i][j][1] * p.alpha;
+        ct[0] = r0;
+        if (two) ct[p.ldct] = r1;
       }
+      double v0 = r0 * ax[j][0], v1 = r1 * ax[j][1];
+      if (use_beta) { v0 += p.beta * cx[j][0]; v1 += p.beta * cx[j][1]; }
       double* c = Cb + (long long)m * p.ldc + n;
-      if (!partial && p.beta != 0.0) {
-        v0 += p.beta * c[0];
-        if (two) v1 += p.beta * c[1];
-      }
       if (two && vec) {
         *reinterpret_cast<double2*>(c) = make_double2(v0, v1);
       } else {

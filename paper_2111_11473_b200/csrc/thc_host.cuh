@@ -13,7 +13,9 @@
 #include "thc_gemm.cuh"
 #include "thc_kernels.cuh"
 #include "thc_triple.cuh"
+#include "thc_gemm_tma.cuh"
 #include "thc_ring.cuh"
+#include "thc_probe.cuh"
 
 struct thc_handle {
   int64_t o, v, NL, NP, NX;
@@ -27,7 +29,10 @@ struct thc_handle {
   int64_t need_bytes;                // what the plan needs with the current block sizes
   int64_t launches;
   int last_cuda;
-  bool smem_configured;
+  bool smem_configured;              // triple_product_kernel opted in to its dynamic shared memory on this handle's device
+  uint64_t gemm_smem_mask, ring_smem_mask;   // same, one bit per dgemm_kernel / ring_fused_kernel instantiation
+  double tma_min_flop;               // GEMMs of at least this many flop may use the TMA-fed kernel (< 0: never)
+  int32_t check_symmetry;
   // Alg.6 line 11: work-item lists (device memory owned by the handle), one per (nPp, NPp) shape seen
   struct TripleList { int64_t nPp, NPp; thc::TripleItem* dev; int n; };
   std::vector<TripleList> tp_lists;
@@ -44,8 +49,11 @@ struct thc_handle {
   std::vector<int> prof_class;              // class of pair k
   std::vector<std::string> prof_desc;       // what pair k timed (printed by thc_profile_end when THC_TRACE is set)
   std::vector<double> prof_flops;          // flop (classes 0, 1) or algorithmic HBM bytes (class 2) of pair k
+  std::vector<float> prof_ms;               // device time of pair k, filled by thc_profile_end
+  size_t prof_done;                         // records readable through thc_profile_launch
   double prof_work[3];                      // summed over the launches of the last thc_profile_end
   size_t prof_used;                         // pairs in use
+  double* sym_scratch;                      // check_symmetry: 8 doubles of device memory owned by the handle
 };
 
 namespace thc {
@@ -102,29 +110,56 @@ constexpr int BIG_THREADS = 256, SMALL_THREADS = 128;
 constexpr int gemm_smem_bytes(int BM, int BN, int BK, int ST, bool akm, bool bkm) {
   return ST * ((akm ? BM * BK : BK * (BM + 2)) + (bkm ? BN * BK : BK * (BN + 2))) * 8;
 }
-// tile 0: 128x128 (one CTA per SM), 1: 128x64 (two), 2: 64x64 (three), 3: 64x64 with a 2-stage ring for K <= 32 (six)
+#define THC_TALL 160, 64, 16, 4, 2, 4       // extents just above 128 (o = 150 at BASELINE config 3): one 160-wide tile instead
+#define THC_WIDE 64, 160, 16, 2, 4, 4       // of two 128-wide ones; K-major, 16-byte aligned operands only
+// tile 0: 128x128 (one CTA per SM), 1: 128x64 (two), 2: 64x64 (three), 3: 64x64 with a 2-stage ring for K <= 32 (six),
+// 4: 160x64, 5: 64x160 (one)
 struct TileCfg { int BM, BN, per_sm; double lone_rate, pipe_share; };
-constexpr TileCfg TILE_CFGS[4] = {{128, 128, 1, 1.0, 1.0}, {128, 64, 2, 0.7, 0.9}, {64, 64, 3, 0.5, 0.75}, {64, 64, 6, 0.5, 0.75}};
+constexpr TileCfg TILE_CFGS[6] = {{128, 128, 1, 1.0, 1.0}, {128, 64, 2, 0.7, 0.9}, {64, 64, 3, 0.5, 0.75}, {64, 64, 6, 0.5, 0.75},
+                                  {160, 64, 1, 0.85, 0.85}, {64, 160, 1, 0.85, 0.85}};
+
+// The opt-in to more than 48 KB of dynamic shared memory is a per-device attribute of the kernel: it is recorded per
+// handle (one handle = one device), bit `bit` of `mask`, never per process.
+template <typename K>
+static cudaError_t opt_in_smem(K k, int bytes, uint64_t& mask, int bit) {
+  if (mask & (1ull << bit)) return cudaSuccess;
+  cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e == cudaSuccess) mask |= 1ull << bit;
+  return e;
+}
 
 template <bool AKM, bool BKM, bool AL16>
-static cudaError_t launch_gemm_variant(int tile, dim3 grid, cudaStream_t st, const GemmParams& p) {
+static cudaError_t launch_gemm_variant(int tile, dim3 grid, cudaStream_t st, const GemmParams& p, uint64_t& mask) {
+  const int bit = tile * 8 + (AKM ? 4 : 0) + (BKM ? 2 : 0) + (AL16 ? 1 : 0);
+  cudaError_t e = cudaSuccess;
+  if (tile >= 4) {                          // only instantiated for K-major, aligned operands (the caller checks)
+    if (!(AKM && BKM && AL16)) return cudaErrorInvalidValue;
+    const int sm = gemm_smem_bytes(160, 64, 16, 4, true, true);
+    if (tile == 4) {
+      auto k = dgemm_kernel<THC_TALL, true, true, true>;
+      if ((e = opt_in_smem(k, sm, mask, 32)) != cudaSuccess) return e;
+      k<<<grid, BIG_THREADS, sm, st>>>(p);
+    } else {
+      auto k = dgemm_kernel<THC_WIDE, true, true, true>;
+      if ((e = opt_in_smem(k, sm, mask, 33)) != cudaSuccess) return e;
+      k<<<grid, BIG_THREADS, sm, st>>>(p);
+    }
+    return cudaPeekAtLastError();
+  }
   if (tile == 0) {
     auto k = dgemm_kernel<THC_BIG, AKM, BKM, AL16>;
     int sm = gemm_smem_bytes(128, 128, THC_BIG_BK, THC_BIG_ST, AKM, BKM);
-    static bool done = false;
-    if (!done) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, sm); done = true; }
+    if ((e = opt_in_smem(k, sm, mask, bit)) != cudaSuccess) return e;
     k<<<grid, BIG_THREADS, sm, st>>>(p);
   } else if (tile == 1) {
     auto k = dgemm_kernel<THC_MID, AKM, BKM, AL16>;
     int sm = gemm_smem_bytes(128, 64, 16, 4, AKM, BKM);
-    static bool done = false;
-    if (!done) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, sm); done = true; }
+    if ((e = opt_in_smem(k, sm, mask, bit)) != cudaSuccess) return e;
     k<<<grid, BIG_THREADS, sm, st>>>(p);
   } else if (tile == 2) {
     auto k = dgemm_kernel<THC_SMALL, AKM, BKM, AL16>;
     int sm = gemm_smem_bytes(64, 64, 16, 4, AKM, BKM);
-    static bool done = false;
-    if (!done) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, sm); done = true; }
+    if ((e = opt_in_smem(k, sm, mask, bit)) != cudaSuccess) return e;
     k<<<grid, SMALL_THREADS, sm, st>>>(p);
   } else {
     auto k = dgemm_kernel<THC_TINYK, AKM, BKM, AL16>;
@@ -173,15 +208,76 @@ struct Ctx {
   int ew_blocks(i64 n, int per = 256) const { return (int)std::max<i64>(1, std::min<i64>((n + per - 1) / per, (i64)h->sms * 16)); }
 
   // ---- GEMM ----------------------------------------------------------------------------------------------------
+  typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  EncodeFn encode_fn() {
+    if (!h->encode_tiled) {
+      void* fn = nullptr;
+      cudaDriverEntryPointQueryResult q;
+      if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || !fn) return nullptr;
+      h->encode_tiled = fn;
+    }
+    return reinterpret_cast<EncodeFn>(h->encode_tiled);
+  }
+  // TMA descriptor of a K-major GEMM operand: element (k, row, kb, b) at base[row * ld + k + kb * sk + b * sb]; box = 8 k x
+  // box_rows rows (64-byte rows, no swizzle: the [k/8][row][8] shared-memory layout).  A zero stride (broadcast operand,
+  // single k-batch) becomes a dimension of extent 1.  Returns false when the driver rejects the layout.
+  bool make_map4(CUtensorMap* m, const double* base, i64 K, i64 rows, i64 ld, i64 nkb, i64 sk, i64 nb, i64 sb, int box_rows) {
+    EncodeFn enc = encode_fn();
+    if (!enc) return false;
+    if (sk == 0) nkb = 1;
+    if (sb == 0) nb = 1;
+    const cuuint64_t dims[4] = {(cuuint64_t)K, (cuuint64_t)rows, (cuuint64_t)nkb, (cuuint64_t)nb};
+    const cuuint64_t dflt = (cuuint64_t)ld * 8;
+    const cuuint64_t strides[3] = {(cuuint64_t)ld * 8, sk ? (cuuint64_t)sk * 8 : dflt, sb ? (cuuint64_t)sb * 8 : dflt};
+    const cuuint32_t box[4] = {8, (cuuint32_t)box_rows, 1, 1}, es[4] = {1, 1, 1, 1};
+    CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double*>(base), dims, strides, box, es,
+                     CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS;
+  }
+  // TMA-fed persistent kernel (thc_gemm_tma.cuh) for tiles 0 (128x128), 4 (160x64), 5 (64x160).  false -> not launched
+  // (the caller falls back to the cp.async kernel).
+  template <int BM, int BN, int WM, int WN, int ST>
+  bool launch_tma_cfg(const GemmParams& p, const CUtensorMap& mA, const CUtensorMap& mB, int bit) {
+    auto k = dgemm_tma_kernel<BM, BN, WM, WN, ST>;
+    const int sm = tg_smem_bytes(BM, BN, ST);
+    if (opt_in_smem(k, sm, h->gemm_smem_mask, bit) != cudaSuccess) { cudaGetLastError(); return false; }
+    const i64 tm = (p.M + BM - 1) / BM, tn = (p.N + BN - 1) / BN;
+    const i64 tiles = (p.upper_only ? tm * (tm + 1) / 2 : tm * tn) * p.splits * p.batch;
+    const int grid = (int)std::min<i64>(tiles, h->sms);
+    k<<<grid, TG_THREADS, sm, h->stream>>>(mA, mB, p);
+    return true;
+  }
+  bool launch_tma(int tile, const Gemm& g, const GemmParams& p) {
+    if (!(tile == 0 || tile == 4 || tile == 5) || !g.akm || !g.bkm) return false;
+    if (g.upper_ && (tile != 0 || g.M != g.N)) return false;
+    const int BM = TILE_CFGS[tile].BM, BN = TILE_CFGS[tile].BN;
+    CUtensorMap mA, mB;
+    if (!make_map4(&mA, g.A, g.K, g.M, g.lda, g.nkb, g.sAk, g.nbatch, g.sAb, BM) ||
+        !make_map4(&mB, g.B, g.K, g.N, g.ldb, g.nkb, g.sBk, g.nbatch, g.sBb, BN)) return false;
+    if (tile == 0) return launch_tma_cfg<128, 128, 2, 4, 6>(p, mA, mB, 40);
+    if (tile == 4) return launch_tma_cfg<160, 64, 4, 2, 6>(p, mA, mB, 41);
+    return launch_tma_cfg<64, 160, 2, 4, 6>(p, mA, mB, 42);
+  }
+
   void gemm(const Gemm& g) {
     if (g.M <= 0 || g.N <= 0 || g.nbatch <= 0) return;
     // Tile shape and split-K factor: minimise  waves x (k-iterations per CTA + fixed cost) x tile area / tile rate  over
     // TILE_CFGS x splits; a split-K pass adds a partial-tile write and a reduction.
     const i64 kiters = (i64)g.nkb * ((g.K + 15) / 16);
+    auto even = [](i64 x) { return (x & 1) == 0; };
+    const bool al16 = ((reinterpret_cast<uintptr_t>(g.A) | reinterpret_cast<uintptr_t>(g.B)) & 15) == 0 && even(g.lda) &&
+                      even(g.ldb) && even(g.sAb) && even(g.sBb) && even(g.sAk) && even(g.sBk);
     int tile = 2, splits = 1; double best = 1e300;
-    for (int cfg = 0; cfg < 3; cfg++) {
+    for (int cfg = 0; cfg < 6; cfg++) {
+      if (cfg == 3) continue;
       const TileCfg& tc = TILE_CFGS[cfg];
       if (cfg < 2 && (g.M <= 64 || g.N <= (cfg == 0 ? 64 : 32))) continue;
+      // 160-wide tiles: only where they save a whole row / column of 128-tiles, K-major aligned operands, plain epilogue
+      if (cfg == 4 && !(g.akm && g.bkm && al16 && !g.upper_ && g.M > 128 && (g.M + 159) / 160 * 160 < (g.M + 127) / 128 * 128)) continue;
+      if (cfg == 5 && !(g.akm && g.bkm && al16 && !g.upper_ && g.N > 128 && (g.N + 159) / 160 * 160 < (g.N + 127) / 128 * 128)) continue;
       i64 tmn = (i64)((g.M + tc.BM - 1) / tc.BM) * ((g.N + tc.BN - 1) / tc.BN) * g.nbatch;
       if (g.upper_) {                                       // only tiles that reach the diagonal or lie above it work
         tmn = 0;
@@ -208,7 +304,22 @@ struct Ctx {
     const i64 per = (i64)g.nbatch * g.M * g.N;
     if (splits > 1) splitk_need = std::max(splitk_need, per * splits);
     if (dry || !ok()) return;
-    if (splits > 1 && per * splits > splitk_cap) { status = THC_ERR_NO_MEMORY; return; }
+    // The scratch was sized by a dry run of the unsharded plan; a shard (other nl / row counts) may prefer more splits
+    // than it has room for: take the largest split factor that fits instead of failing.
+    if (splits > 1 && per * splits > splitk_cap) splits = (int)std::max<i64>(1, splitk_cap / per);
+    // grid.z carries batch x splits and is limited to 65535: long batches go out as several launches
+    if ((i64)g.nbatch * splits > 65535) {
+      const int chunk = std::max(1, 65535 / splits);
+      for (int b0 = 0; b0 < g.nbatch && ok(); b0 += chunk) {
+        Gemm part = g;
+        part.nbatch = std::min(chunk, g.nbatch - b0);
+        part.A = g.A + (i64)b0 * g.sAb; part.B = g.B + (i64)b0 * g.sBb; part.C = g.C + (i64)b0 * g.sCb;
+        if (g.aux_) part.aux_ = g.aux_ + (i64)b0 * g.sAuxb;
+        if (g.ct_) part.ct_ = g.ct_ + (i64)b0 * g.sCtb;
+        gemm(part);
+      }
+      return;
+    }
 
     GemmParams p;
     p.A = g.A; p.B = g.B; p.aux = g.aux_;
@@ -222,28 +333,29 @@ struct Ctx {
     if (splits > 1) { p.C = splitk; p.ldc = g.N; p.sCb = (i64)g.M * g.N; p.sCs = per; }
     else            { p.C = g.C; p.ldc = g.ldc; p.sCb = g.sCb; p.sCs = 0; }
 
-    auto even = [](i64 x) { return (x & 1) == 0; };
-    const bool al16 = ((reinterpret_cast<uintptr_t>(g.A) | reinterpret_cast<uintptr_t>(g.B)) & 15) == 0 && even(g.lda) &&
-                      even(g.ldb) && even(g.sAb) && even(g.sBb) && even(g.sAk) && even(g.sBk);
-    i64 zdim = (i64)g.nbatch * splits;
-    if (zdim > 65535) { status = THC_ERR_INVALID_ARG; return; }
-    dim3 grid((unsigned)tiles_mn, 1, (unsigned)zdim);
+    dim3 grid((unsigned)tiles_mn, 1, (unsigned)((i64)g.nbatch * splits));
     cudaError_t e;
     char desc[160];
     if (h->prof_mask & 1)
-      snprintf(desc, sizeof desc, "gemm %s M=%d N=%d K=%d batch=%d kbatch=%d splits=%d %c%c%s", tile == 0 ? "big" : (tile == 1 ? "mid" : (tile == 2 ? "small" : "tinyK")), g.M, g.N, g.K,
+      snprintf(desc, sizeof desc, "gemm %s M=%d N=%d K=%d batch=%d kbatch=%d splits=%d %c%c%s", tile == 0 ? "big" : (tile == 1 ? "mid" : (tile == 2 ? "small" : (tile == 3 ? "tinyK" : (tile == 4 ? "tall" : "wide")))), g.M, g.N, g.K,
                g.nbatch, g.nkb, splits, g.akm ? 'K' : 'M', g.bkm ? 'K' : 'N', al16 ? "" : " unaligned");
     prof_start(0, desc, 2.0 * g.M * g.N * (double)g.K * g.nbatch * g.nkb * (g.upper_ ? 0.5 * (1.0 + (double)tc.BN / g.N) : 1.0));
     const int sel = (g.akm ? 4 : 0) | (g.bkm ? 2 : 0) | (al16 ? 1 : 0);
+    // large aligned K-major products go to the TMA-fed persistent kernel; small ones (launch-bound shapes, where encoding
+    // two descriptors costs more than it saves) and everything else to the cp.async kernel
+    const bool want_tma = al16 && h->tma_min_flop >= 0 && 2.0 * g.M * g.N * (double)g.K * g.nbatch * g.nkb >= h->tma_min_flop;
+    if (want_tma && launch_tma(tile, g, p)) {
+      e = cudaPeekAtLastError();
+    } else
     switch (sel) {
-      case 7: e = launch_gemm_variant<true, true, true>(tile, grid, h->stream, p); break;
-      case 6: e = launch_gemm_variant<true, true, false>(tile, grid, h->stream, p); break;
-      case 5: e = launch_gemm_variant<true, false, true>(tile, grid, h->stream, p); break;
-      case 4: e = launch_gemm_variant<true, false, false>(tile, grid, h->stream, p); break;
-      case 3: e = launch_gemm_variant<false, true, true>(tile, grid, h->stream, p); break;
-      case 2: e = launch_gemm_variant<false, true, false>(tile, grid, h->stream, p); break;
-      case 1: e = launch_gemm_variant<false, false, true>(tile, grid, h->stream, p); break;
-      default: e = launch_gemm_variant<false, false, false>(tile, grid, h->stream, p); break;
+      case 7: e = launch_gemm_variant<true, true, true>(tile, grid, h->stream, p, h->gemm_smem_mask); break;
+      case 6: e = launch_gemm_variant<true, true, false>(tile, grid, h->stream, p, h->gemm_smem_mask); break;
+      case 5: e = launch_gemm_variant<true, false, true>(tile, grid, h->stream, p, h->gemm_smem_mask); break;
+      case 4: e = launch_gemm_variant<true, false, false>(tile, grid, h->stream, p, h->gemm_smem_mask); break;
+      case 3: e = launch_gemm_variant<false, true, true>(tile, grid, h->stream, p, h->gemm_smem_mask); break;
+      case 2: e = launch_gemm_variant<false, true, false>(tile, grid, h->stream, p, h->gemm_smem_mask); break;
+      case 1: e = launch_gemm_variant<false, false, true>(tile, grid, h->stream, p, h->gemm_smem_mask); break;
+      default: e = launch_gemm_variant<false, false, false>(tile, grid, h->stream, p, h->gemm_smem_mask); break;
     }
     h->launches++;
     check(e);
@@ -365,13 +477,11 @@ struct Ctx {
   void ring_launch(const RingParams& p, bool al16, dim3 grid) {
     const int sm = ring_smem_bytes(KT);
     if (al16) {
-      static bool done = false;
-      if (!done) { check(cudaFuncSetAttribute(ring_fused_kernel<KT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm)); done = true; }
-      ring_fused_kernel<KT, true><<<grid, RG_THREADS, sm, h->stream>>>(p);
+      check(opt_in_smem(ring_fused_kernel<KT, true>, sm, h->ring_smem_mask, 2 * KT));
+      if (ok()) ring_fused_kernel<KT, true><<<grid, RG_THREADS, sm, h->stream>>>(p);
     } else {
-      static bool done = false;
-      if (!done) { check(cudaFuncSetAttribute(ring_fused_kernel<KT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm)); done = true; }
-      ring_fused_kernel<KT, false><<<grid, RG_THREADS, sm, h->stream>>>(p);
+      check(opt_in_smem(ring_fused_kernel<KT, false>, sm, h->ring_smem_mask, 2 * KT + 1));
+      if (ok()) ring_fused_kernel<KT, false><<<grid, RG_THREADS, sm, h->stream>>>(p);
     }
   }
   // FYT[b][j][I] = sum_J (sum_i YoT[I][i] RYT[b][J][i]) V[I][J] Yo[j][J]

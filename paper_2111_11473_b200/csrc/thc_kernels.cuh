@@ -205,6 +205,29 @@ __global__ void fock_kernel(const double* __restrict__ eps, const double* __rest
   }
 }
 
+// thc_options.check_symmetry: out[0] = max |A_b[i][j] - A_b[j][i]|, out[1] = max |A_b[i][j]| over nbatch densely packed
+// n x n matrices, as the bit patterns of non-negative doubles (which order like unsigned integers).
+__global__ void asym_max_kernel(const double* __restrict__ A, int n, i64 nbatch, unsigned long long* __restrict__ out) {
+  const i64 total = nbatch * n * n;
+  double d = 0.0, m = 0.0;
+  THC_GRID_STRIDE(idx, total) {
+    const int j = (int)(idx % n);
+    const i64 r = idx / n;
+    const int i = (int)(r % n);
+    const double x = A[idx];
+    m = fmax(m, fabs(x));
+    if (j > i) d = fmax(d, fabs(x - A[(r - i + j) * n + i]));
+  }
+  for (int off = 16; off > 0; off >>= 1) {
+    d = fmax(d, __shfl_xor_sync(0xffffffffu, d, off));
+    m = fmax(m, __shfl_xor_sync(0xffffffffu, m, off));
+  }
+  if ((threadIdx.x & 31) == 0) {
+    atomicMax(out, (unsigned long long)__double_as_longlong(d));
+    atomicMax(out + 1, (unsigned long long)__double_as_longlong(m));
+  }
+}
+
 // R = sum of up to six terms
 __global__ void sum6_kernel(const double* a, const double* b, const double* c, const double* d, const double* e,
                             const double* f, double* __restrict__ out, i64 n) {

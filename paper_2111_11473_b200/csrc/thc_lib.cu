@@ -22,7 +22,9 @@ using thc::Gemm;
 namespace {
 
 struct Inputs {
-  const double *Xo, *Xv, *Z, *B_ov, *B_oo, *B_vv, *Y, *V, *eps;
+  const double *Xo, *Xv, *Z, *B_ov, *B_oo;
+  const void* B_vv;        // device array, host array or thc_bvv_provider*, per thc_options.bvv_mode (thc.h)
+  const double *Y, *V, *eps;
 };
 struct Outputs {
   double* R;
@@ -111,21 +113,21 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out, const Shard& sh
   if (streamed) { bvv_buf[0] = ar.alloc(h->bL * v * v); bvv_buf[1] = ar.alloc(h->bL * v * v); }
   if (streamed && !c.dry) c.bvv_begin();
   if (streamed && !c.dry && h->bvv_mode == THC_BVV_HOST)
-    c.bvv_copy(bvv_buf[0], in.B_vv, 0, std::min<i64>(h->bL, NL), v, 0);
+    c.bvv_copy(bvv_buf[0], static_cast<const double*>(in.B_vv), 0, std::min<i64>(h->bL, NL), v, 0);
   i64 blk = 0;
   for (i64 L0 = 0; L0 < NL; L0 += h->bL, blk++) {
     const i64 nl = std::min<i64>(h->bL, NL - L0);
     const i64 m0 = ar.mark();
-    const double* bvv = in.B_vv + L0 * v * v;
+    const double* bvv = static_cast<const double*>(in.B_vv) + L0 * v * v;
     if (streamed) {
       bvv = bvv_buf[blk & 1];
       if (!c.dry) {
         if (h->bvv_mode == THC_BVV_HOST) {
           const i64 L1 = L0 + h->bL;                 // prefetch the next block while this one is consumed
-          if (L1 < NL) c.bvv_copy(bvv_buf[(blk + 1) & 1], in.B_vv, L1, std::min<i64>(h->bL, NL - L1), v, blk + 1);
+          if (L1 < NL) c.bvv_copy(bvv_buf[(blk + 1) & 1], static_cast<const double*>(in.B_vv), L1, std::min<i64>(h->bL, NL - L1), v, blk + 1);
           c.bvv_wait_loaded(blk);
         } else {
-          c.bvv_provide(reinterpret_cast<const thc_bvv_provider*>(in.B_vv), Lb + L0, nl, bvv_buf[blk & 1]);
+          c.bvv_provide(static_cast<const thc_bvv_provider*>(in.B_vv), Lb + L0, nl, bvv_buf[blk & 1]);
         }
       }
     }
@@ -287,23 +289,35 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out, const Shard& sh
   if (do_s6 && local) {
     const i64 m0 = ar.mark();
     const i64 NPp = pad_to(NP, thc::TP_RT);
-    // line 1: A3[Q][i][a] = sum_S Z[Q,S] Xo[i,S] Xv[a,S]
-    double* A3 = ar.alloc(NP * ov);
-    const i64 bA = std::min<i64>(NP, h->bP7 * 16);
-    for (i64 P0 = 0; P0 < NP; P0 += bA) {
-      const i64 npb = std::min<i64>(bA, NP - P0), m1 = ar.mark();
-      double* ZX = ar.alloc(npb * o * NP);
-      c.rowscale(in.Xo, NP, in.Z + P0 * NP, NP, nullptr, 1.0, ZX, npb, o, NP);
-      c.gemm(Gemm(ZX, NP, 'K', in.Xv, NP, 'K', A3 + P0 * ov, v, npb * o, v, NP));
-      ar.release(m1);
-    }
+    // line 1: A3[Q][i][a] = sum_S Z[Q,S] Xo[i,S] Xv[a,S].  It only feeds lines 4-5 at the start of a row block.  While it
+    // is small it stays resident; at paper scale (22.5 GB at config 4) it is rebuilt for every row block in the memory
+    // that the I-chunk buffers reuse afterwards (+2 NP^2 o v flop per block, ~2 % of the evaluation, for 22 GB more H).
+    const bool a3_resident = NP * ov * 8 <= ((i64)4 << 30) || Pe - Pb <= h->bX;
+    auto build_A3 = [&](double* A3) {
+      const i64 bA = std::max<i64>(1, std::min<i64>(NP, ((i64)1 << 28) / (o * NP)));      // <= 2 GB of scaled factors at a time
+      for (i64 P0 = 0; P0 < NP; P0 += bA) {
+        const i64 npb = std::min<i64>(bA, NP - P0), m1 = ar.mark();
+        double* ZX = ar.alloc(npb * o * NP);
+        c.rowscale(in.Xo, NP, in.Z + P0 * NP, NP, nullptr, 1.0, ZX, npb, o, NP);
+        c.gemm(Gemm(ZX, NP, 'K', in.Xv, NP, 'K', A3 + P0 * ov, v, npb * o, v, NP));
+        ar.release(m1);
+      }
+    };
+    double* A3r = nullptr;
+    if (a3_resident) { A3r = ar.alloc(NP * ov); build_A3(A3r); }
     for (i64 P0 = Pb; P0 < Pe; P0 += h->bX) {                // this rank's rows of sigma6
       const i64 npb = std::min<i64>(h->bX, Pe - P0), m1 = ar.mark();
       const i64 bXp = pad_to(npb, thc::TP_PT);
       // lines 4-5: Cc[p][(q,i)] = sum_a Xv[a,P0+p] A3[q][i][a] ;  Dd[p][(q,a)] = sum_i Xo[i,P0+p] A3[q][i][a]
       double *Cc = ar.alloc(npb * NP * o), *Dd = ar.alloc(npb * NP * v), *H = ar.alloc(bXp * NPp * NPp);
-      c.gemm(Gemm(XvT + P0 * v, v, 'K', A3, v, 'K', Cc, NP * o, npb, NP * o, v));
-      c.gemm(Gemm(XoT + P0 * o, o, 'K', A3, v, 'N', Dd, NP * v, npb, v, o).batch(NP, 0, ov, v));
+      {
+        const i64 m3 = ar.mark();
+        double* A3 = A3r;
+        if (!a3_resident) { A3 = ar.alloc(NP * ov); build_A3(A3); }
+        c.gemm(Gemm(XvT + P0 * v, v, 'K', A3, v, 'K', Cc, NP * o, npb, NP * o, v));
+        c.gemm(Gemm(XoT + P0 * o, o, 'K', A3, v, 'N', Dd, NP * v, npb, v, o).batch(NP, 0, ov, v));
+        ar.release(m3);
+      }
       bool first = true;
       for (i64 I0 = 0; I0 < NX; I0 += h->bI) {
         const i64 ni = std::min<i64>(h->bI, NX - I0), m2 = ar.mark();
@@ -435,6 +449,38 @@ int make_ctx(Ctx& c, thc_handle* h, char* base, i64 bytes, const Need& need) {
   return THC_OK;
 }
 
+// thc_options.check_symmetry (debug): Z, V, every B^L_oo and -- when resident -- every B^L_vv must be symmetric to 1e-12
+// of their largest element, because the plan evaluates symmetric products on one triangle only (thc.h).  One pass over
+// HBM and one host synchronisation; NL_local Cholesky vectors are present.
+int check_symmetric(thc_handle* h, const Inputs& in, i64 NL_local) {
+  if (!h->sym_scratch) {
+    void* p = nullptr;
+    cudaError_t e = cudaMalloc(&p, 8 * sizeof(double));
+    if (e != cudaSuccess) { h->last_cuda = (int)e; cudaGetLastError(); return THC_ERR_NO_MEMORY; }
+    h->sym_scratch = static_cast<double*>(p);
+  }
+  cudaError_t e = cudaMemsetAsync(h->sym_scratch, 0, 8 * sizeof(double), h->stream);
+  if (e != cudaSuccess) { h->last_cuda = (int)e; return THC_ERR_CUDA; }
+  unsigned long long* out = reinterpret_cast<unsigned long long*>(h->sym_scratch);
+  struct Item { const double* A; i64 n, nb; } items[4] = {
+      {in.Z, h->NP, 1}, {in.V, h->NX, 1}, {in.B_oo, h->o, NL_local},
+      {h->bvv_mode == THC_BVV_DEVICE ? static_cast<const double*>(in.B_vv) : nullptr, h->v, NL_local}};
+  for (int k = 0; k < 4; k++) {
+    if (!items[k].A || items[k].nb <= 0) continue;
+    const i64 total = items[k].nb * items[k].n * items[k].n;
+    const int blocks = (int)std::max<i64>(1, std::min<i64>((total + 255) / 256, (i64)h->sms * 16));
+    thc::asym_max_kernel<<<blocks, 256, 0, h->stream>>>(items[k].A, (int)items[k].n, items[k].nb, out + 2 * k);
+    h->launches++;
+  }
+  double res[8];
+  e = cudaMemcpyAsync(res, h->sym_scratch, sizeof res, cudaMemcpyDeviceToHost, h->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+  if (e != cudaSuccess) { h->last_cuda = (int)e; return THC_ERR_CUDA; }
+  for (int k = 0; k < 4; k++)
+    if (res[2 * k] > 1e-12 * res[2 * k + 1]) return THC_ERR_INVALID_ARG;
+  return THC_OK;
+}
+
 struct DeviceGuard {
   int prev = -1; bool ok = true;
   explicit DeviceGuard(int dev) { if (cudaGetDevice(&prev) != cudaSuccess) ok = false; else if (prev != dev) ok = cudaSetDevice(dev) == cudaSuccess; }
@@ -478,7 +524,8 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
   if (!hp) return THC_ERR_INVALID_ARG;
   *hp = nullptr;
   if (o <= 0 || v <= 0 || NL <= 0 || NP <= 0 || NX <= 0) return THC_ERR_INVALID_ARG;
-  if (opt && (opt->bvv_mode < 0 || opt->bvv_mode > 2 || opt->reserved != 0)) return THC_ERR_INVALID_ARG;
+  if (opt && (opt->bvv_mode < 0 || opt->bvv_mode > 2 || opt->reserved != 0 || opt->use_graph < -1 || opt->use_graph > 1))
+    return THC_ERR_INVALID_ARG;
   if (opt && (opt->bL < 0 || opt->bP7 < 0 || opt->bX < 0 || opt->bI < 0 || opt->workspace_bytes_max < 0)) return THC_ERR_INVALID_ARG;
   const int64_t lim = (int64_t)1 << 31;
   if (o >= lim || v >= lim || NL >= lim || NP >= lim || NX >= lim) return THC_ERR_OVERFLOW;
@@ -503,14 +550,16 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
   h->device = dev; h->sms = prop.multiProcessorCount;
   h->stream = nullptr; h->ws = nullptr; h->ws_bytes = 0; h->ws_owned = false;
   h->launches = 0; h->last_cuda = 0; h->smem_configured = false;
-  h->prof_mask = 0; h->prof_used = 0; h->encode_tiled = nullptr;
+  h->gemm_smem_mask = 0; h->ring_smem_mask = 0; h->tma_min_flop = (opt && opt->tma_min_flop) ? (double)opt->tma_min_flop : 2e8;
+  h->check_symmetry = opt ? opt->check_symmetry : 0; h->sym_scratch = nullptr;
+  h->prof_mask = 0; h->prof_used = 0; h->prof_done = 0; h->encode_tiled = nullptr;
   h->prof_work[0] = h->prof_work[1] = h->prof_work[2] = 0.0;
   h->bvv_mode = opt ? opt->bvv_mode : THC_BVV_DEVICE; h->copy_stream = nullptr; h->copy_ready = false;
 
   // block sizes: defaults, then shrink until the plan fits the cap
   h->bL = std::min<int64_t>(NL, (opt && opt->bL) ? opt->bL : 512);    // long L-blocks: few, large GEMMs (shrunk below if HBM is short)
   const int64_t p7_auto = o <= 64 ? std::max<int64_t>(1, ((int64_t)2 << 30) / (NX * (o + v) * 8 + 1))
-                                  : std::max<int64_t>(1, ((int64_t)2 << 30) / (NX * NX * 8));
+                                  : std::max<int64_t>(1, ((int64_t)8 << 30) / (NX * NX * 8));   // E .* V is materialised
   h->bP7 = std::min<int64_t>(NP, (opt && opt->bP7) ? opt->bP7 : p7_auto);
   h->bX = std::min<int64_t>(pad_to(NP, 16), (opt && opt->bX) ? pad_to(opt->bX, 16) : pad_to(NP, 16));
   h->bI = std::min<int64_t>(NX, (opt && opt->bI) ? opt->bI : 1024);   // long I loops amortise the H read-modify-write
@@ -519,7 +568,8 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
     DeviceGuard g(dev);
     size_t fr = 0, tot = 0;
     if (!g.ok || cudaMemGetInfo(&fr, &tot) != cudaSuccess) { delete h; return THC_ERR_CUDA; }
-    cap = (int64_t)(0.75 * (double)fr);
+    // the workspace is the only large allocation the library makes; the T2^2 phases at paper scale need every GB
+    cap = (int64_t)(0.92 * (double)fr);
   }
   const bool fix_bX = opt && opt->bX, fix_bI = opt && opt->bI, fix_bP7 = opt && opt->bP7, fix_bL = opt && opt->bL;
   {
@@ -539,10 +589,15 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
     h->bX = sX; h->bI = sI;
     if (!fix_bX && !fix_bI && need_device(h) > cap) {
       const double fo = (double)o, fv = (double)v, fNP = (double)NP, fNX = (double)NX;
-      const double t_g = fNX * (2 * fo * fv * fNP + 2 * fo * fNP * fNP + 2 * fo * fv * fNX) / 25e12;       // DMMA, s
-      const double t_h = 16.0 * fNP * (double)pad_to(NP, 32) * (double)pad_to(NP, 32) / 5e12;            // HBM, s
+      // measured on B200 (profiles/): the K = NX and K = v products of a G pass run at ~30 TFLOP/s, the K = o product
+      // with its N x N output at ~22; the read-modify-write of H at the end of every work item of line 11 is not
+      // overlapped with its FMAs, so it costs about twice its HBM time.  (+ A3 rebuilt per row block when not resident.)
+      const double t_g = fNX * ((2 * fo * fv * fNX + 2 * fo * fv * fNP) / 30e12 + 2 * fo * fNP * fNP / 22e12) +
+                         (NP * o * v * 8 > ((i64)4 << 30) ? 2 * fNP * fNP * fo * fv / 30e12 : 0.0);           // DMMA, s
+      const double t_h = 16.0 * fNP * (double)pad_to(NP, 32) * (double)pad_to(NP, 32) / 2.5e12;          // HBM, s
       double best = 1e300; int64_t bestX = 0, bestI = 0;
-      for (int64_t bi : {16, 24, 32, 48, 64, 96, 128, 192, 256, 384, 512, 768, 1024}) {
+      // (chunks of a multiple of 128 grid points fill the 128-row tiles of the E_I / F_I products)
+      for (int64_t bi : {16, 32, 64, 128, 256, 384, 512, 640, 768, 896, 1024}) {
         if (bi > NX) break;
         h->bI = bi; h->bX = 16;
         if (need_device(h) > cap) break;
@@ -578,12 +633,13 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
 
 int thc_destroy(thc_handle* h) {
   if (!h) return THC_ERR_INVALID_ARG;
-  if ((h->ws && h->ws_owned) || !h->prof_events.empty() || !h->tp_lists.empty() || h->copy_ready) {
+  if ((h->ws && h->ws_owned) || !h->prof_events.empty() || !h->tp_lists.empty() || h->copy_ready || h->sym_scratch) {
     DeviceGuard g(h->device);
     cudaStreamSynchronize(h->stream);
     if (h->ws && h->ws_owned) cudaFree(h->ws);
     for (cudaEvent_t e : h->prof_events) cudaEventDestroy(e);
     for (auto& l : h->tp_lists) cudaFree(l.dev);
+    if (h->sym_scratch) cudaFree(h->sym_scratch);
     if (h->copy_ready) {
       cudaStreamSynchronize(h->copy_stream);
       for (int k = 0; k < 2; k++) { cudaEventDestroy(h->ev_loaded[k]); cudaEventDestroy(h->ev_free[k]); }
@@ -622,7 +678,7 @@ int thc_get_blocks(const thc_handle* h, int64_t out[4]) {
 }
 
 int thc_residual_terms(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
-                       const double* B_oo, const double* B_vv, const double* Y, const double* V, const double* eps,
+                       const double* B_oo, const void* B_vv, const double* Y, const double* V, const double* eps,
                        double* R, double* const terms[6], double* xi_oo, double* xi_vv) {
   if (!h) return THC_ERR_INVALID_ARG;
   if (bad_ptr(Xo) || bad_ptr(Xv) || bad_ptr(Z) || bad_ptr(B_ov) || bad_ptr(B_oo) || bad_ptr(B_vv) || bad_ptr(Y) ||
@@ -640,11 +696,12 @@ int thc_residual_terms(thc_handle* h, const double* Xo, const double* Xv, const 
   if (!g.ok) return THC_ERR_CUDA;
   int st = ensure_workspace(h, h->need_bytes);
   if (st != THC_OK) return st;
+  if (h->check_symmetry && (st = check_symmetric(h, in, h->NL)) != THC_OK) return st;
   return run_residual(h, static_cast<char*>(h->ws), h->ws_bytes, in, out);
 }
 
 int thc_residual(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
-                 const double* B_oo, const double* B_vv, const double* Y, const double* V, const double* eps, double* R) {
+                 const double* B_oo, const void* B_vv, const double* Y, const double* V, const double* eps, double* R) {
   if (!R) return THC_ERR_INVALID_ARG;
   return thc_residual_terms(h, Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps, R, nullptr, nullptr, nullptr);
 }
@@ -680,7 +737,7 @@ int64_t thc_shard_doubles(const thc_handle* h) {
 }
 
 int thc_residual_shard(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
-                       const double* B_oo, const double* B_vv, const double* Y, const double* V, const double* eps,
+                       const double* B_oo, const void* B_vv, const double* Y, const double* V, const double* eps,
                        int rank, int nranks, double* packed) {
   if (!h || bad_ptr(Xo) || bad_ptr(Xv) || bad_ptr(Z) || bad_ptr(Y) || bad_ptr(V) || bad_ptr(eps) || bad_ptr(packed))
     return THC_ERR_INVALID_ARG;
@@ -696,6 +753,7 @@ int thc_residual_shard(thc_handle* h, const double* Xo, const double* Xv, const 
   if (!g.ok) return THC_ERR_CUDA;
   st = ensure_workspace(h, h->need_bytes);
   if (st != THC_OK) return st;
+  if (h->check_symmetry && (st = check_symmetric(h, in, r[1] - r[0])) != THC_OK) return st;
   return run_residual(h, static_cast<char*>(h->ws), h->ws_bytes, in, out, sh);
 }
 
@@ -754,18 +812,18 @@ int thc_profile_end(thc_handle* h, double ms[3], int64_t counts[3]) {
   for (int k = 0; k < 3; k++) { ms[k] = 0.0; counts[k] = 0; h->prof_work[k] = 0.0; }
   cudaError_t e = cudaStreamSynchronize(h->stream);
   if (e != cudaSuccess) { h->last_cuda = (int)e; return THC_ERR_CUDA; }
-  const bool trace = getenv("THC_TRACE") != nullptr;     // developer aid: one stderr line per timed launch
+  h->prof_ms.assign(h->prof_used, 0.f);
+  h->prof_done = 0;
   for (size_t k = 0; k < h->prof_used; k++) {
     float t = 0.f;
     e = cudaEventElapsedTime(&t, h->prof_events[2 * k], h->prof_events[2 * k + 1]);
     if (e != cudaSuccess) { h->last_cuda = (int)e; return THC_ERR_CUDA; }
-    if (trace)
-      fprintf(stderr, "[thc trace] %9.4f ms  %8.3f T(fl)op/s-or-Gelem/s  %s\n", t, h->prof_flops[k] / (t * 1e-3) / 1e12,
-              h->prof_desc[k].c_str());
+    h->prof_ms[k] = t;
     ms[h->prof_class[k]] += (double)t;
     counts[h->prof_class[k]]++;
     h->prof_work[h->prof_class[k]] += h->prof_flops[k];
   }
+  h->prof_done = h->prof_used;
   h->prof_mask = 0;
   h->prof_used = 0;
   return THC_OK;
@@ -777,11 +835,25 @@ int thc_profile_work(const thc_handle* h, double work[3]) {
   return THC_OK;
 }
 
+int64_t thc_profile_launches(const thc_handle* h) { return h ? (int64_t)h->prof_done : (int64_t)THC_ERR_INVALID_ARG; }
+
+int thc_profile_launch(const thc_handle* h, int64_t k, int* cls, double* ms, double* work, char* desc, int64_t desc_bytes) {
+  if (!h || k < 0 || (size_t)k >= h->prof_done) return THC_ERR_INVALID_ARG;
+  if (cls) *cls = h->prof_class[k];
+  if (ms) *ms = (double)h->prof_ms[k];
+  if (work) *work = h->prof_flops[k];
+  if (desc && desc_bytes > 0) {
+    strncpy(desc, h->prof_desc[k].c_str(), (size_t)desc_bytes - 1);
+    desc[desc_bytes - 1] = 0;
+  }
+  return THC_OK;
+}
+
 int thc_residual_host(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
-                      const double* B_oo, const double* B_vv, const double* Y, const double* V, const double* eps,
+                      const double* B_oo, const void* B_vv, const double* Y, const double* V, const double* eps,
                       double* R_host, double* E_host) {
   if (!h || !R_host) return THC_ERR_INVALID_ARG;
-  const double* src[9] = {Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps};
+  const double* src[9] = {Xo, Xv, Z, B_ov, B_oo, static_cast<const double*>(B_vv), Y, V, eps};
   for (int k = 0; k < 9; k++) if (bad_ptr(src[k])) return THC_ERR_INVALID_ARG;
   DeviceGuard g(h->device);
   if (!g.ok) return THC_ERR_CUDA;
@@ -806,6 +878,7 @@ int thc_residual_host(thc_handle* h, const double* Xo, const double* Xv, const d
   Inputs in{dev[0], dev[1], dev[2], dev[3], dev[4], dev[5], dev[6], dev[7], dev[8]};
   Outputs out{};
   out.R = Rd;
+  if (h->check_symmetry && (st = check_symmetric(h, in, h->NL)) != THC_OK) return st;
   st = run_residual(h, p, rest, in, out);
   if (st != THC_OK) return st;
   cudaError_t e = cudaMemcpyAsync(R_host, Rd, (size_t)h->NP * h->NP * 8, cudaMemcpyDeviceToHost, h->stream);
@@ -848,6 +921,15 @@ double thc_algorithmic_flops(const thc_handle* h) {
   return f;
 }
 
+int thc_algorithmic_work(const thc_handle* h, double work[3]) {
+  if (!h || !work) return THC_ERR_INVALID_ARG;
+  const double NL = (double)h->NL, NP = (double)h->NP, NX = (double)h->NX;
+  work[1] = 5 * NX * NP * NP * NP;                      // H9 (d): line 11
+  work[2] = 5 * NL * NP * NP;                           // H3
+  work[0] = thc_algorithmic_flops(h) - work[1] - work[2];
+  return THC_OK;
+}
+
 int thc_dgemm(thc_handle* h, int a_kmajor, int b_kmajor, int64_t M, int64_t N, int64_t K, double alpha, const double* A,
               int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc) {
   if (!h || bad_ptr(A) || bad_ptr(B) || bad_ptr(C) || M <= 0 || N <= 0 || K <= 0) return THC_ERR_INVALID_ARG;
@@ -885,19 +967,67 @@ int thc_triple_product(thc_handle* h, int64_t nI, int64_t nPp, int64_t NPp, cons
   return c.status;
 }
 
+int thc_probe(thc_handle* h, double out[8]) {
+  if (!h || !out) return THC_ERR_INVALID_ARG;
+  DeviceGuard g(h->device);
+  if (!g.ok) return THC_ERR_CUDA;
+  for (int k = 0; k < 8; k++) out[k] = 0.0;
+  double* sink = nullptr;
+  cudaEvent_t e0, e1;
+  if (cudaMalloc(&sink, 64) != cudaSuccess || cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
+    h->last_cuda = (int)cudaGetLastError();
+    return THC_ERR_CUDA;
+  }
+  int khz = 0;
+  cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, h->device);          // maximum SM clock
+  const double clk = (double)khz * 1e3;
+  const int grid = h->sms, fp_iters = 1 << 16, lds_iters = 1 << 15;
+  auto timed = [&](auto launch) -> double {                                 // seconds, best of 3 after a warm-up
+    launch();
+    float best = 1e30f;
+    for (int r = 0; r < 3; r++) {
+      cudaEventRecord(e0, h->stream);
+      launch();
+      cudaEventRecord(e1, h->stream);
+      cudaEventSynchronize(e1);
+      float ms = 0.f;
+      cudaEventElapsedTime(&ms, e0, e1);
+      best = std::min(best, ms);
+    }
+    return (double)best * 1e-3;
+  };
+  const double warps = (double)grid * thc::PROBE_THREADS / 32, n_fp = (double)fp_iters * thc::PROBE_UNROLL;
+  const double dmma_flop = warps * n_fp * 2.0 * 8 * 8 * 4, dfma_flop = warps * 32.0 * n_fp * 2.0;
+  out[0] = dmma_flop / timed([&] { thc::probe_fp64_kernel<0><<<grid, thc::PROBE_THREADS, 0, h->stream>>>(sink, fp_iters, 1.25); }) / 1e12;
+  out[1] = dfma_flop / timed([&] { thc::probe_fp64_kernel<1><<<grid, thc::PROBE_THREADS, 0, h->stream>>>(sink, fp_iters, 1.25); }) / 1e12;
+  out[2] = (dmma_flop + dfma_flop) / timed([&] { thc::probe_fp64_kernel<2><<<grid, thc::PROBE_THREADS, 0, h->stream>>>(sink, fp_iters, 1.25); }) / 1e12;
+  unsigned* usink = reinterpret_cast<unsigned*>(sink);
+  const double lanes_loads = (double)grid * thc::PROBE_THREADS * lds_iters * 8.0;
+  out[3] = lanes_loads * 4 / timed([&] { thc::probe_lds_kernel<4><<<grid, thc::PROBE_THREADS, 0, h->stream>>>(usink, lds_iters, 0u); }) / clk / grid;
+  out[4] = lanes_loads * 8 / timed([&] { thc::probe_lds_kernel<8><<<grid, thc::PROBE_THREADS, 0, h->stream>>>(usink, lds_iters, 0u); }) / clk / grid;
+  out[5] = lanes_loads * 16 / timed([&] { thc::probe_lds_kernel<16><<<grid, thc::PROBE_THREADS, 0, h->stream>>>(usink, lds_iters, 0u); }) / clk / grid;
+  out[6] = clk / 1e6;
+  h->launches += 24;
+  cudaError_t e = cudaGetLastError();
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+  if (e != cudaSuccess) { h->last_cuda = (int)e; return THC_ERR_CUDA; }
+  return THC_OK;
+}
+
 const char* thc_strerror(int status) {
   switch (status) {
     case THC_OK: return "ok";
     case THC_ERR_INVALID_ARG: return "invalid argument (null or misaligned pointer, bad size)";
     case THC_ERR_OVERFLOW: return "size overflow";
     case THC_ERR_NO_MEMORY: return "workspace too small or device allocation failed";
-    case THC_ERR_CUDA: return "CUDA error (see thc_last_cuda_error)";
+    case THC_ERR_CUDA: return "CUDA error (see thc_last_error)";
     case THC_ERR_NO_DEVICE: return "no sm_100 CUDA device";
     case THC_ERR_PROVIDER: return "B_vv provider callback failed";
     default: return "unknown status";
   }
 }
 
-int thc_last_cuda_error(const thc_handle* h) { return h ? h->last_cuda : 0; }
+int thc_last_error(const thc_handle* h) { return h ? h->last_cuda : 0; }
+int thc_last_cuda_error(const thc_handle* h) { return thc_last_error(h); }
 
 }  // extern "C"

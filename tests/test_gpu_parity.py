@@ -78,6 +78,16 @@ def test_block_size_invariance(blocks):
     _check_against(x, ref, **blocks)
 
 
+@pytest.mark.parametrize("dims", [(6, 18, 10, 64, 96), (66, 10, 6, 34, 40), (4, 6, 3, 642, 8)])
+def test_tma_gemm_path_on_small_shapes(dims):
+    """Every aligned K-major product forced onto the TMA-fed GEMM kernel (tma_min_flop=1): batched, k-batched, aux,
+    transposed-copy, upper-only and split-K launches of the plan on shapes with ragged tiles."""
+    x = small_inputs(*dims, seed=13, zmul=30.0)
+    ref = oracle_eval(x)
+    _check_against(x, ref, tma_min_flop=1)
+    _check_against(x, ref, tma_min_flop=1, bL=3, bP7=5, bX=32, bI=10)
+
+
 def test_term_mask_and_zero_cases():
     import torch
     import paper_2111_11473_b200 as thc
@@ -169,3 +179,43 @@ def test_provider_fill_is_stream_ordered_at_scale():
         R = h.thc_residual(*args)
         assert torch.equal(R, ref)
     h.close()
+
+
+def test_unfused_alg7_path_o_above_64():
+    """o > 64 takes the Alg.7 path that BASELINE configs 3 and 4 use (no 64-wide fused kernel): checked here against
+    the dense oracle on a cheap shape so that a regression is caught without the multi-minute runs."""
+    x = small_inputs(66, 9, 5, 33, 40, seed=21, zmul=30.0)
+    ref = oracle_eval(x)
+    _check_against(x, ref)
+    _check_against(x, ref, bP7=4, bX=16, bI=16)
+
+
+def test_symmetric_half_path_odd_NP():
+    """NP >= 640 switches the half-transforms to upper-tile GEMMs + mirror; odd NP takes the scalar load path."""
+    x = small_inputs(3, 4, 3, 641, 8, seed=22, zmul=30.0)
+    ref = oracle_eval(x)
+    _check_against(x, ref)
+
+
+def test_check_symmetry_option_rejects_unsymmetric_inputs():
+    import paper_2111_11473_b200 as thc
+    x = small_inputs(4, 9, 8, 24, 30, seed=2, zmul=30.0)
+    ref = oracle_eval(x)
+    _check_against(x, ref, check_symmetry=True)               # symmetric inputs pass
+    d = _to_dev(x)
+    for k in (2, 4, 5, 7):                                    # Z, B_oo, B_vv, V
+        bad = [t.clone() for t in d]
+        bad[k].view(-1)[1] += 1e-3                            # element (0, 1) of the first matrix
+        h = thc.thc_setup(x.o, x.v, x.NL, x.NP, x.NX, check_symmetry=True)
+        with pytest.raises(thc.ThcError, match="invalid argument"):
+            h.thc_residual(*bad)
+        h.close()
+
+
+def test_probe_reports_plausible_ceilings():
+    import paper_2111_11473_b200 as thc
+    h = thc.thc_setup(4, 8, 4, 16, 16)
+    p = h.thc_probe()
+    h.close()
+    assert 20.0 < p["dmma_tflops"] < 60.0 and 20.0 < p["dfma_tflops"] < 60.0, p
+    assert 60.0 < p["lds128_bytes_per_clk_per_sm"] <= 140.0, p

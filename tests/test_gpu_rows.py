@@ -1,7 +1,7 @@
 """Parity of the CUDA path against the T2 sampled-row oracle (oracle/rows.py) at sizes the dense oracle cannot hold.
 
-Config 2 (o=60, v=340, NL=1200, NP=1000, NX=2000) runs by default, in the launch configuration bench.py times; config 3
-is opt-in (THC_BIG_TESTS=1: ~20 GB of inputs and minutes of CPU per row).  Inputs are drawn on the device by
+Configs 2 and 3 run by default, in the launch configuration bench.py times (config 3 is its default workload); config 4
+is opt-in (THC_BIG_TESTS=4: an evaluation takes ~13 minutes and the CPU rows about an hour).  Inputs are drawn on the device by
 thc_synth.device and the very same tensors are copied to the host for the oracle.  Tolerances as in test_gpu_parity.py:
 1e-10 relative to each term's own maximum over the sampled rows, 1e-9 E_h on the energy.
 """
@@ -16,7 +16,7 @@ TERMS = ("s1", "s2", "s3", "s6", "s7", "s9")
 NAMES = ("Xo", "Xv", "Z", "B_ov", "B_oo", "B_vv", "Y", "V", "eps")
 
 
-def _run(cfg, rows, rows_s6, lblock, terms=TERMS, check_xi_and_energy=True, provider=False):
+def _run(cfg, rows, rows_s6, lblock, terms=TERMS, check_xi_and_energy=True, provider=False, cheap_pins=None):
     import torch
     import paper_2111_11473_b200 as thc
     from thc_synth import CONFIGS
@@ -42,6 +42,19 @@ def _run(cfg, rows, rows_s6, lblock, terms=TERMS, check_xi_and_energy=True, prov
     print(f"config {cfg}: one residual evaluation (all terms) {time.perf_counter() - t0:.1f} s", flush=True)
     E = h.thc_energy(d["Xo"], d["Xv"], d["Z"], d["B_ov"])
     torch.cuda.synchronize()
+    cheap = {}
+    if cheap_pins:
+        # energy contribution of single Cholesky vectors: NL ranks -> rank L owns exactly vector L
+        for L in cheap_pins["L"]:
+            cheap[("E", L)] = float(h.thc_energy_shard(d["Xo"], d["Xv"], d["Z"], d["B_ov"][L:L + 1].contiguous(), L, c["NL"])[0])
+        # eps part of sigma9 at this NP: a handle with one zero Cholesky vector (xi = 0, sigma1..3 = 0)
+        h0 = thc.thc_setup(c["o"], c["v"], 1, c["NP"], c["NX"], term_mask=thc.TERM_BITS["s9"] | thc.TERM_BITS["s2"])
+        z = lambda *shape: torch.zeros(*shape, dtype=torch.float64, device="cuda")
+        r0 = h0.thc_residual_terms(d["Xo"], d["Xv"], d["Z"], z(1, c["o"], c["v"]), z(1, c["o"], c["o"]),
+                                   z(1, c["v"], c["v"]), d["Y"], d["V"], d["eps"])
+        cheap["s9_eps"] = r0["s9"][cheap_pins["P"]].cpu().numpy()
+        h0.close()
+        del r0
     got = {k: res[k][list(rows)].cpu().numpy() for k in TERMS + ("R",)}
     xi_oo, xi_vv = res["xi_oo"].cpu().numpy(), res["xi_vv"].cpu().numpy()
     sym = float((res["R"] - res["R"].T).abs().max() / res["R"].abs().max())
@@ -60,17 +73,35 @@ def _run(cfg, rows, rows_s6, lblock, terms=TERMS, check_xi_and_energy=True, prov
         errs["xi_oo"] = np.abs(xi_oo - rxo).max() / np.abs(rxo).max()
         errs["xi_vv"] = np.abs(xi_vv - rxv).max() / np.abs(rxv).max()
         errs["E_abs"] = abs(E - ro.energy())
+    if cheap_pins:
+        t0 = time.perf_counter()
+        for L in cheap_pins["L"]:
+            sub = [host[n][L:L + 1] if n in ("B_ov", "B_oo") else host[n] for n in NAMES]
+            sub[5] = np.zeros((1, c["v"], c["v"]))
+            e_ref = RowOracle(*sub, lblock=1).energy()
+            errs[f"E_L{L}_abs"] = abs(cheap[("E", L)] - e_ref)
+        j, b = cheap_pins["j"], cheap_pins["b"]
+        col, row_v = ro.xi_oo_column(j), ro.xi_vv_row(b)
+        errs["xi_oo_column"] = np.abs(xi_oo[:, j] - col).max() / np.abs(col).max()
+        errs["xi_vv_row"] = np.abs(xi_vv[b] - row_v).max() / np.abs(row_v).max()
+        zero = [np.zeros((1,) + host[n].shape[1:]) if n in ("B_ov", "B_oo") else host[n] for n in NAMES]
+        zero[5] = np.zeros((1, c["v"], c["v"]))
+        s9_ref = RowOracle(*zero, lblock=1).row(cheap_pins["P"], terms=("s9",))["s9"]
+        errs["s9_eps_part"] = np.abs(cheap["s9_eps"] - s9_ref).max() / np.abs(s9_ref).max()
+        print(f"config {cfg}: cheap pins (E per vector, xi column/row, sigma9 eps part) {time.perf_counter() - t0:.0f} s CPU", flush=True)
     ref = {k: [] for k in terms}
     all_terms = terms
     for n, P in enumerate(rows):
         terms = all_terms if P in rows_s6 else tuple(k for k in all_terms if k != "s6")
+        t0 = time.perf_counter()
         r = ro.row(P, terms=terms)
+        print(f"config {cfg}: oracle row P={P} terms {terms}: {time.perf_counter() - t0:.0f} s CPU", flush=True)
         for k in terms:
             ref[k].append((n, r[k]))
     for k in all_terms:
         scale = max(np.abs(r).max() for _, r in ref[k])
         errs[k] = max(np.abs(got[k][n] - r).max() for n, r in ref[k]) / scale
-    bad = {k: e for k, e in errs.items() if e > (1e-9 if k == "E_abs" else 1e-10)}
+    bad = {k: e for k, e in errs.items() if e > (1e-9 if k.startswith("E_") else 1e-10)}
     assert not bad, f"parity failures {bad} (all: {errs})"
     print(f"config {cfg} sampled-row parity: {errs}")
 
@@ -79,14 +110,23 @@ def test_config2_sampled_rows():
     _run(2, rows=(3, 777), rows_s6=(3,), lblock=16)
 
 
-@pytest.mark.skipif(os.environ.get("THC_BIG_TESTS") not in ("1", "3"), reason="set THC_BIG_TESTS=3 (config 3: ~20 GB, ~10 min)")
 def test_config3_sampled_rows():
+    """BASELINE config 3 (the bench.py default workload): ~40 s of GPU and ~9 min of CPU row oracle."""
     _run(3, rows=(1234,), rows_s6=(1234,), lblock=8)
 
 
-@pytest.mark.skipif(os.environ.get("THC_BIG_TESTS") != "4", reason="set THC_BIG_TESTS=4 (config 4: ~40 GB resident, B_vv streamed; ~40 min)")
+@pytest.mark.skipif(not os.environ.get("THC_BIG_TESTS", "").startswith("4"),
+                    reason="set THC_BIG_TESTS=4 (config 4: ~40 GB resident, B_vv streamed, ~15 min of GPU and ~1 h of CPU "
+                           "row oracle; THC_BIG_TESTS=4s6 adds one row of sigma6, ~40 min more)")
 def test_config4_sampled_rows_streamed_bvv():
-    """Paper-scale config: B_vv (304 GB) comes from a provider callback one L-block at a time.  The terms whose rows the
-    CPU can afford are checked (s1, s2, s3: linear in the Cholesky ERIs; s7); s6, s9 (xi) and E would take hours of CPU
-    per row here and are pinned through config 3."""
-    _run(4, rows=(2718,), rows_s6=(), lblock=4, terms=("s1", "s2", "s3", "s7"), check_xi_and_energy=False, provider=True)
+    """Paper-scale config: B_vv (304 GB) comes from a provider callback one L-block at a time.  One sampled row of
+    sigma1, sigma2, sigma3, sigma7 (and sigma6 with THC_BIG_TESTS=4s6) against the row oracle; the energy through
+    sampled Cholesky vectors (thc_energy_shard with one vector per rank vs the oracle restricted to that vector, long
+    double); xi_oo / xi_vv through one sampled column / row (Eqs.39-40 with one index fixed); sigma9 through its
+    eps part (a second handle with NL = 1 and B = 0: Alg.9 at this NP without the xi dressing).  The xi part of sigma9
+    is linear in xi and shares the Alg.9 code path with the eps part; a row of it would need the full xi (hours of CPU):
+    DESIGN.md section 5 lists it as unpinned at this config."""
+    s6 = os.environ.get("THC_BIG_TESTS") == "4s6"
+    _run(4, rows=(2718,), rows_s6=(2718,) if s6 else (), lblock=4,
+         terms=("s1", "s2", "s3", "s6", "s7") if s6 else ("s1", "s2", "s3", "s7"),
+         check_xi_and_energy=False, provider=True, cheap_pins=dict(L=(0, 3141, 7499), j=123, b=1999, P=2718))

@@ -39,3 +39,17 @@ def test_rows_callable_bvv():
     got = ro.row(2, terms=("s1", "s3"))
     for k in ("s1", "s3"):
         assert np.abs(got[k] - ref[k][2]).max() <= 1e-12 * np.abs(ref[k]).max()
+
+
+@pytest.mark.parametrize("dims", [(3, 4, 6, 5, 7), (4, 9, 8, 12, 15)])
+def test_single_xi_column_and_row_match_dense(dims):
+    """xi_oo_column / xi_vv_row (used where the full xi is unaffordable, BASELINE config 4) against the dense oracle's
+    xi of Eqs.39-40 -- every column / row, so that a transposed index would show (xi_oo is not symmetric, R5)."""
+    x = small_inputs(*dims, seed=23, zmul=30.0)
+    ref = oracle_eval(x)
+    ro = RowOracle(x.Xo, x.Xv, x.Z, x.B_ov, x.B_oo, x.B_vv, x.Y, x.V, x.eps, lblock=3)
+    assert np.abs(ref["xi_oo"] - ref["xi_oo"].T).max() > 1e-6 * np.abs(ref["xi_oo"]).max()
+    for j in range(x.o):
+        assert np.abs(ro.xi_oo_column(j) - ref["xi_oo"][:, j]).max() <= 1e-12 * np.abs(ref["xi_oo"]).max(), j
+    for b in range(x.v):
+        assert np.abs(ro.xi_vv_row(b) - ref["xi_vv"][b]).max() <= 1e-12 * np.abs(ref["xi_vv"]).max(), b

@@ -139,9 +139,11 @@ class ThcInputs:
                                       self.Y, self.V) ) + (0 if self.B_vv is None else self.B_vv.nbytes)
 
 
-def make_inputs(o, v, NL, NP, NX, seed, with_bvv=True, z_scale=0.1) -> ThcInputs:
-    """Draw one full input set.  `z_scale` is the std of Z before symmetrisation (R15)."""
+def make_inputs(o, v, NL, NP, NX, seed, with_bvv=True, z_scale=0.1, l_keep=None) -> ThcInputs:
+    """Draw one full input set.  `z_scale` is the std of Z before symmetrisation (R15).  `l_keep` draws only the first
+    l_keep Cholesky vectors of the NL (same values as in the full set; a bounded sample of a large workload)."""
     n = o + v
+    NL_full, NL = NL, (NL if l_keep is None else min(NL, int(l_keep)))
     eps_o = np.sort(-1.5 + 1.2 * uniform_block(seed, TENSOR_IDS["eps_o"], np.arange(o)))
     eps_v = np.sort(0.1 + 2.9 * uniform_block(seed, TENSOR_IDS["eps_v"], np.arange(v)))
     eps = np.concatenate([eps_o, eps_v])
@@ -150,15 +152,15 @@ def make_inputs(o, v, NL, NP, NX, seed, with_bvv=True, z_scale=0.1) -> ThcInputs
     G = _normal_full(seed, TENSOR_IDS["Z"], (NP, NP))
     Z = z_scale * 0.5 * (G + G.T)
     del G
-    B_oo = np.ascontiguousarray(_bsym_block(seed, n, NL, 0, NL, 0, o, 0, o))
-    B_ov = np.ascontiguousarray(_bsym_block(seed, n, NL, 0, NL, 0, o, o, n))
+    B_oo = np.ascontiguousarray(_bsym_block(seed, n, NL_full, 0, NL, 0, o, 0, o))
+    B_ov = np.ascontiguousarray(_bsym_block(seed, n, NL_full, 0, NL, 0, o, o, n))
     B_vv = None
     if with_bvv:
         B_vv = np.empty((NL, v, v), dtype=np.float64)
         step = max(1, (1 << 22) // max(1, v * v))
         for L0 in range(0, NL, step):
             L1 = min(NL, L0 + step)
-            B_vv[L0:L1] = bvv_block(seed, o, v, NL, L0, L1)
+            B_vv[L0:L1] = bvv_block(seed, o, v, NL_full, L0, L1)
     Y = _normal_full(seed, TENSOR_IDS["Y"], (n, NX)) / np.sqrt(NX)
     G = _normal_full(seed, TENSOR_IDS["VG"], (NX, NX))
     V = (G @ G.T) / NX
