@@ -133,6 +133,17 @@ int thc_residual_terms(thc_handle* h, const double* Xo, const double* Xv, const 
                        const double* B_oo, const void* B_vv, const double* Y, const double* V,
                        const double* eps, double* R, double* const terms[6], double* xi_oo, double* xi_vv);
 
+/* Rank-reduced working variables (Eqs.13-14 l.116-120, Eq.22 l.178-181): with the orthogonalised CP factor
+ * tau[NR][NP] (tau~^{PW}, P < NR) and the symmetric core T[NR][NR] in the semi-unitary basis,
+ *     Z = tau^T T tau                (the THC-basis core T^{WX} of Eq.22),
+ *     R_rr = tau R(Z) tau^T          (the amplitude equations projected with U~ = sum_W y y tau~, Eqs.6 and 14).
+ * Device pointers, asynchronous.  Z_out[NP][NP] (optional, may be NULL) receives Z.  Needs thc_workspace_bytes_rr(h, NR)
+ * bytes of workspace (the residual's plus Z, R and one NR x NP temporary).  The other arguments are thc_residual's. */
+int64_t thc_workspace_bytes_rr(const thc_handle* h, int64_t NR);
+int thc_residual_rr(thc_handle* h, int64_t NR, const double* tau, const double* T, const double* Xo, const double* Xv,
+                    const double* B_ov, const double* B_oo, const void* B_vv, const double* Y, const double* V,
+                    const double* eps, double* R_rr, double* Z_out);
+
 /* Correlation energy E = sum_L [ 2 a^L.Z.a^L - sum_PQ Z_PQ E^L_PQ E^L_QP ] (factorised form of
  * sum (2t - t^x)(ia|jb); a^L, E^L from Alg.8 l.5-6).  Device pointers in, one double written to the HOST
  * address E_host; synchronises the stream.                                                             */
@@ -208,11 +219,10 @@ int thc_dgemm(thc_handle* h, int a_kmajor, int b_kmajor, int64_t M, int64_t N, i
 
 /* Alg.6 line 11 (l.714) alone, for tests and roofline measurement:
  * H[p][q][r] (+)= sum_I (E[I][p][q] F[I][p][r] + E[I][p][r] F[I][p][q]) G[I][q][r]
- * E, F: [nI][nPp][NPp], G, GT: [nI][NPp][NPp] with GT[I][q][r] = G[I][r][q] (the caller supplies both orientations;
- * the kernel reads the mirrored block from GT), H: [nPp][NPp][NPp]; NPp a multiple of 32, nPp of 16 (padded extents;
+ * E, F: [nI][nPp][NPp], G: [nI][NPp][NPp], H: [nPp][NPp][NPp]; NPp a multiple of 32, nPp of 16 (padded extents;
  * padded entries are computed from whatever the padding holds and must be ignored).  All pointers 16-byte aligned. */
 int thc_triple_product(thc_handle* h, int64_t nI, int64_t nPp, int64_t NPp, const double* E, const double* F,
-                       const double* G, const double* GT, double* H, int accumulate);
+                       const double* G, double* H, int accumulate);
 
 /* Measured FP64 / shared-memory ceilings of the handle's device (synchronous; ~0.3 s).  MEASURED_PEAKS.json has no
  * FP64 entry, so the rooflines of DESIGN.md section 7 rest on these:  out[0] issue rate of the FP64 tensor instruction

@@ -160,3 +160,56 @@ def omega_bruteforce(t, eri, eps, o, v):
         sign, det = r
         omega[i, a, j, b] = sign * hpsi.get(det, 0.0) - t[i, a, j, b] * e_tot
     return omega, e_tot - e_ref
+
+
+# ---- with singles: <mu| exp(-T) H exp(T) |Phi0>, T = T1 + T2 (no CC formula, no T1-dressing identity) --------------------
+def apply_T1(vec, t1, o, v):
+    """(sum_ia t1[i,a] E_ai) |vec>."""
+    out = {}
+    for det, c in vec.items():
+        for i in range(o):
+            for a in range(v):
+                if t1[i, a] == 0.0:
+                    continue
+                for s in (0, 1):
+                    r = _apply_string(det, [("a", 2 * i + s), ("c", 2 * (o + a) + s)])
+                    if r is not None:
+                        _vec_add(out, r[1], c * t1[i, a] * r[0])
+    return out
+
+
+def _exp_T(vec, t1, t, o, v, sign):
+    """exp(sign * (T1 + T2)) |vec> by its (terminating) power series."""
+    out, term, n = dict(vec), dict(vec), 0
+    while term:
+        n += 1
+        nxt = apply_T1(term, t1, o, v)
+        for d, c in apply_T2(term, t, o, v).items():
+            _vec_add(nxt, d, c)
+        term = {d: sign * c / n for d, c in nxt.items() if c != 0.0}
+        for d, c in term.items():
+            _vec_add(out, d, c)
+        if n > 4 * (o + v):
+            raise RuntimeError("series did not terminate")
+    return out
+
+
+def residuals_bruteforce_t1(t1, t, eri, eps, o, v):
+    """(sigma[i,a], Omega[i,a,j,b]) = <mu| exp(-T) H exp(T) |Phi0> for the alpha single and the alpha-beta double
+    excitation bras; h is fixed by the BARE Fock matrix being diag(eps), `eri` are the bare (pq|rs)."""
+    n = o + v
+    h = np.diag(np.asarray(eps, dtype=float)).copy()
+    for i in range(o):
+        h -= 2.0 * eri[:, :, i, i] - eri[:, i, i, :]
+    phi0 = (1 << (2 * o)) - 1
+    psi = _exp_T({phi0: 1.0}, t1, t, o, v, +1.0)
+    r = _exp_T(apply_H(psi, h, eri, n), t1, t, o, v, -1.0)
+    sigma = np.zeros((o, v))
+    for i, a in itertools.product(range(o), range(v)):
+        sg, det = _apply_string(phi0, [("a", 2 * i), ("c", 2 * (o + a))])
+        sigma[i, a] = sg * r.get(det, 0.0)
+    omega = np.zeros((o, v, o, v))
+    for i, a, j, b in itertools.product(range(o), range(v), range(o), range(v)):
+        sg, det = _apply_string(phi0, [("a", 2 * j + 1), ("c", 2 * (o + b) + 1), ("a", 2 * i), ("c", 2 * (o + a))])
+        omega[i, a, j, b] = sg * r.get(det, 0.0)
+    return sigma, omega

@@ -24,7 +24,8 @@ SYMBOLS = ("thc_setup", "thc_destroy", "thc_workspace_bytes", "thc_workspace_byt
            "thc_energy_device", "thc_residual_host", "thc_profile_begin", "thc_profile_end", "thc_profile_work", "thc_kernel_launches", "thc_algorithmic_flops", "thc_dgemm",
            "thc_triple_product", "thc_strerror", "thc_last_cuda_error", "thc_last_error", "thc_shard_range",
            "thc_shard_doubles", "thc_residual_shard", "thc_residual_finish", "thc_energy_shard",
-           "thc_profile_launches", "thc_profile_launch", "thc_algorithmic_work", "thc_probe")
+           "thc_profile_launches", "thc_profile_launch", "thc_algorithmic_work", "thc_probe", "thc_workspace_bytes_rr",
+           "thc_residual_rr")
 
 TERM_NAMES = ("s1", "s2", "s3", "s6", "s7", "s9")
 TERM_BITS = dict(s1=1, s2=2, s3=4, s6=8, s7=16, s9=32)
@@ -110,13 +111,16 @@ def lib() -> ctypes.CDLL:
     L.thc_algorithmic_work.argtypes = [VP, ctypes.POINTER(D * 3)]
     L.thc_last_error.argtypes = [VP]
     L.thc_probe.argtypes = [VP, ctypes.POINTER(D * 8)]
+    L.thc_workspace_bytes_rr.argtypes = [VP, I64]
+    L.thc_workspace_bytes_rr.restype = I64
+    L.thc_residual_rr.argtypes = [VP, I64] + [P] * 12
     L.thc_residual_host.argtypes = [VP] + [P] * 10 + [ctypes.POINTER(D)]
     L.thc_kernel_launches.argtypes = [VP]
     L.thc_kernel_launches.restype = I64
     L.thc_algorithmic_flops.argtypes = [VP]
     L.thc_algorithmic_flops.restype = D
     L.thc_dgemm.argtypes = [VP, ctypes.c_int, ctypes.c_int, I64, I64, I64, D, P, I64, P, I64, D, P, I64]
-    L.thc_triple_product.argtypes = [VP, I64, I64, I64, P, P, P, P, P, ctypes.c_int]
+    L.thc_triple_product.argtypes = [VP, I64, I64, I64, P, P, P, P, ctypes.c_int]
     L.thc_shard_range.argtypes = [I64, I64, ctypes.c_int, ctypes.c_int, ctypes.POINTER(I64 * 4)]
     L.thc_shard_doubles.argtypes = [VP]
     L.thc_shard_doubles.restype = I64
@@ -273,6 +277,22 @@ class Thc:
                                         _dev_ptr(res["xi_oo"], "xi_oo"), _dev_ptr(res["xi_vv"], "xi_vv")), self._h)
         return res
 
+    def thc_residual_rr(self, tau, T, Xo, Xv, B_ov, B_oo, B_vv, Y, V, eps, want_Z=False):
+        """R_rr [NR, NR] = tau R(Z) tau^T with Z = tau^T T tau (rank-reduced working variables; device tensors)."""
+        import torch
+        NR = int(tau.shape[0])
+        o, v, NL, NP, NX = self.o, self.v, self.NL, self.NP, self.NX
+        self._prepare(int(lib().thc_workspace_bytes_rr(self._h, NR)))
+        kw = dict(dtype=torch.float64, device=self._device)
+        R_rr = torch.empty(NR, NR, **kw)
+        Z = torch.empty(NP, NP, **kw) if want_Z else None
+        _check(lib().thc_residual_rr(
+            self._h, NR, _dev_ptr(tau, "tau", NR * NP), _dev_ptr(T, "T", NR * NR), _dev_ptr(Xo, "Xo", o * NP),
+            _dev_ptr(Xv, "Xv", v * NP), _dev_ptr(B_ov, "B_ov", NL * o * v), _dev_ptr(B_oo, "B_oo", NL * o * o),
+            self._bvv_ptr(B_vv, _dev_ptr), _dev_ptr(Y, "Y", (o + v) * NX), _dev_ptr(V, "V", NX * NX),
+            _dev_ptr(eps, "eps", o + v), _dev_ptr(R_rr, "R_rr"), _dev_ptr(Z, "Z") if want_Z else None), self._h)
+        return (R_rr, Z) if want_Z else R_rr
+
     def thc_energy(self, Xo, Xv, Z, B_ov) -> float:
         self._prepare(self.workspace_bytes)
         o, v, NL, NP = self.o, self.v, self.NL, self.NP
@@ -411,10 +431,10 @@ class Thc:
         _check(lib().thc_dgemm(self._h, int(a_kmajor), int(b_kmajor), M, N, K, alpha, _dev_ptr(A, "A"), lda,
                                _dev_ptr(B, "B"), ldb, beta, _dev_ptr(C, "C"), ldc), self._h)
 
-    def thc_triple_product(self, nI, nPp, NPp, E, F, G, GT, H, accumulate):
+    def thc_triple_product(self, nI, nPp, NPp, E, F, G, H, accumulate):
         self._prepare(self.workspace_bytes)
         _check(lib().thc_triple_product(self._h, nI, nPp, NPp, _dev_ptr(E, "E", nI * nPp * NPp),
-                                        _dev_ptr(F, "F", nI * nPp * NPp), _dev_ptr(G, "G", nI * NPp * NPp), _dev_ptr(GT, "GT", nI * NPp * NPp),
+                                        _dev_ptr(F, "F", nI * nPp * NPp), _dev_ptr(G, "G", nI * NPp * NPp),
                                         _dev_ptr(H, "H", nPp * NPp * NPp), int(accumulate)), self._h)
 
 

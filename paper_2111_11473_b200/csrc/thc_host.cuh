@@ -54,6 +54,15 @@ struct thc_handle {
   double prof_work[3];                      // summed over the launches of the last thc_profile_end
   size_t prof_used;                         // pairs in use
   double* sym_scratch;                      // check_symmetry: 8 doubles of device memory owned by the handle
+  // CUDA graphs for launch-bound shapes (thc_options.use_graph): one cached executable graph per entry point (0 = residual,
+  // 1 = energy), valid while every pointer of the call, the workspace and the stream stay the same.  The first call
+  // with a new key runs eagerly (it also does the one-time opt-ins and work-list uploads), the second one is captured on
+  // cap_stream (the caller's stream may be the legacy default stream, which cannot be captured) and launched, later ones
+  // only launch.
+  struct GraphSlot { std::vector<uintptr_t> key; int seen = 0; cudaGraphExec_t exec = nullptr; int64_t launches = 0; };
+  GraphSlot graph[2];
+  bool graph_on;
+  cudaStream_t cap_stream;
 };
 
 namespace thc {
@@ -582,23 +591,22 @@ struct Ctx {
     h->tp_lists.push_back(l);
     return &h->tp_lists.back();
   }
-  void triple_product(const double* E, const double* F, const double* G, const double* GT, double* H, i64 nI, i64 nPp, i64 NPp, int accumulate) {
+  void triple_product(const double* E, const double* F, const double* G, double* H, i64 nI, i64 nPp, i64 NPp, int accumulate) {
     if (dry || !ok()) return;
     if (!h->smem_configured) {
       check(cudaFuncSetAttribute(triple_product_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TP_SMEM_BYTES));
       h->smem_configured = true;
     }
     const thc_handle::TripleList* list = triple_items(nPp, NPp);
-    CUtensorMap mE, mF, mG, mGT;
-    if (!list || !make_map3(&mE, E, NPp, nPp, nI) || !make_map3(&mF, F, NPp, nPp, nI) || !make_map3(&mG, G, NPp, NPp, nI) ||
-        !make_map3(&mGT, GT, NPp, NPp, nI)) return;
+    CUtensorMap mE, mF, mG;
+    if (!list || !make_map3(&mE, E, NPp, nPp, nI) || !make_map3(&mF, F, NPp, nPp, nI) || !make_map3(&mG, G, NPp, NPp, nI)) return;
     TripleParams p;
     p.H = H; p.items = list->dev; p.n_items = list->n;
     p.nI = (int)nI; p.nPp = (int)nPp; p.NPp = (int)NPp; p.accumulate = accumulate;
     const int grid = std::min(list->n, h->sms);
     if (((i64)(list->n + grid - 1) / grid) * nI >= ((i64)1 << 31)) { status = THC_ERR_OVERFLOW; return; }
     prof_start(1, "triple_product", 5.0 * nI * nPp * (double)NPp * NPp);
-    triple_product_kernel<<<grid, TP_THREADS, TP_SMEM_BYTES, h->stream>>>(mE, mF, mG, mGT, p);
+    triple_product_kernel<<<grid, TP_THREADS, TP_SMEM_BYTES, h->stream>>>(mE, mF, mG, p);
     launched();
     prof_stop(1);
   }

@@ -322,19 +322,19 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out, const Shard& sh
       for (i64 I0 = 0; I0 < NX; I0 += h->bI) {
         const i64 ni = std::min<i64>(h->bI, NX - I0), m2 = ar.mark();
         // line 2/7: BI[I][i][a] = sum_J V[I,J] Yo[i,J] Yv[a,J]
-        double *VY = ar.alloc(ni * o * NX), *BI = ar.alloc(ni * ov), *GXT = ar.alloc(ni * NP * o), *Gt = ar.alloc(ni * NPp * NPp), *GtT = ar.alloc(ni * NPp * NPp);
+        double *VY = ar.alloc(ni * o * NX), *BI = ar.alloc(ni * ov), *GXT = ar.alloc(ni * NP * o), *Gt = ar.alloc(ni * NPp * NPp);
         double *Eb = ar.alloc(ni * bXp * NPp), *Fb = ar.alloc(ni * bXp * NPp);
         c.rowscale(Yo, NX, in.V + I0 * NX, NX, nullptr, 1.0, VY, ni, o, NX);
         c.gemm(Gemm(VY, NX, 'K', Yv, NX, 'K', BI, v, ni * o, v, NX));
         // line 10: G_I[q][r] = sum_ia Xo[i,q] Xv[a,r] BI[I][i][a]
         c.gemm(Gemm(XvT, v, 'K', BI, v, 'K', GXT, o, NP, o, v).batch(ni, 0, ov, NP * o));
-        // (the epilogue also writes the transpose GtT_I[q][r] = G_I[r][q], read by the mirrored half of line 11)
-        c.gemm(Gemm(XoT, o, 'K', GXT, o, 'K', Gt, NPp, NP, NP, o).batch(ni, 0, NP * o, NPp * NPp).transposed_copy(GtT, NPp, NPp * NPp));
+        // (line 11 reads the mirrored half G_I[r][q] from the same array: no transposed copy)
+        c.gemm(Gemm(XoT, o, 'K', GXT, o, 'K', Gt, NPp, NP, NP, o).batch(ni, 0, NP * o, NPp * NPp));
         // lines 8-9: E_I[p][q] = sum_i Cc[p][(q,i)] Yo[i,I] ;  F_I[p][r] = sum_a Dd[p][(r,a)] Yv[a,I]
         c.gemm(Gemm(YoT + I0 * o, o, 'K', Cc, o, 'K', Eb, bXp * NPp, ni, NP, o).batch(npb, 0, NP * o, NPp));
         c.gemm(Gemm(YvT + I0 * v, v, 'K', Dd, v, 'K', Fb, bXp * NPp, ni, NP, v).batch(npb, 0, NP * v, NPp));
         // line 11
-        c.triple_product(Eb, Fb, Gt, GtT, H, ni, bXp, NPp, first ? 0 : 1);
+        c.triple_product(Eb, Fb, Gt, H, ni, bXp, NPp, first ? 0 : 1);
         first = false;
         ar.release(m2);
       }
@@ -496,6 +496,58 @@ int run_residual(thc_handle* h, char* base, i64 bytes, const Inputs& in, const O
   if (c.ar.overflow) return THC_ERR_NO_MEMORY;
   return c.status;
 }
+
+// Run `body` (which enqueues one evaluation on h->stream) either directly or through the cached CUDA graph of `slot`
+// (thc_handle::GraphSlot).  `key` = every pointer the evaluation depends on.
+template <typename Body>
+int run_maybe_graphed(thc_handle* h, int slot, std::vector<uintptr_t> key, Body body) {
+  const bool eligible = h->graph_on && h->bvv_mode == THC_BVV_DEVICE && h->prof_mask == 0;
+  if (!eligible) return body();
+  key.push_back(reinterpret_cast<uintptr_t>(h->ws));
+  key.push_back((uintptr_t)h->ws_bytes);
+  key.push_back(reinterpret_cast<uintptr_t>(h->stream));
+  thc_handle::GraphSlot& g = h->graph[slot];
+  if (g.key != key) {
+    if (g.exec) { cudaGraphExecDestroy(g.exec); g.exec = nullptr; }
+    g.key = key;
+    g.seen = 0;
+  }
+  g.seen++;
+  if (g.seen == 1) return body();                       // eager: one-time opt-ins, work lists, descriptor entry point
+  if (!g.exec) {
+    if (!h->cap_stream && cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+      cudaGetLastError();
+      h->graph_on = false;
+      return body();
+    }
+    cudaStream_t user = h->stream;
+    const int64_t l0 = h->launches;
+    h->stream = h->cap_stream;
+    cudaGraph_t graph = nullptr;
+    cudaError_t e = cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal);
+    int st = THC_OK;
+    if (e == cudaSuccess) {
+      st = body();
+      e = cudaStreamEndCapture(h->cap_stream, &graph);
+    }
+    h->stream = user;
+    if (e == cudaSuccess && st == THC_OK) e = cudaGraphInstantiate(&g.exec, graph, 0);
+    if (graph) cudaGraphDestroy(graph);
+    if (e != cudaSuccess || st != THC_OK || !g.exec) {  // capture not possible here: fall back to plain launches for good
+      cudaGetLastError();
+      g.exec = nullptr;
+      h->graph_on = false;
+      h->launches = l0;
+      return body();
+    }
+    g.launches = h->launches - l0;
+    h->launches = l0;
+  }
+  cudaError_t e = cudaGraphLaunch(g.exec, h->stream);
+  if (e != cudaSuccess) { h->last_cuda = (int)e; return THC_ERR_CUDA; }
+  h->launches += g.launches;
+  return THC_OK;
+}
 int run_energy(thc_handle* h, char* base, i64 bytes, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
                double* E_host, double* E_dev, i64 NL_local = -1) {
   Need need = dry_energy(h);
@@ -553,7 +605,12 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
   h->gemm_smem_mask = 0; h->ring_smem_mask = 0; h->tma_min_flop = (opt && opt->tma_min_flop) ? (double)opt->tma_min_flop : 2e8;
   h->check_symmetry = opt ? opt->check_symmetry : 0; h->sym_scratch = nullptr;
   h->prof_mask = 0; h->prof_used = 0; h->prof_done = 0; h->encode_tiled = nullptr;
-  h->prof_work[0] = h->prof_work[1] = h->prof_work[2] = 0.0;
+  h->cap_stream = nullptr;
+  {
+    const int ug = opt ? opt->use_graph : -1;
+    const bool resident = (opt ? opt->bvv_mode : THC_BVV_DEVICE) == THC_BVV_DEVICE;
+    h->graph_on = resident && (ug == 1 || (ug == -1 && thc_algorithmic_flops(h) < 2e10));   // auto: launch-bound shapes only
+  }
   h->bvv_mode = opt ? opt->bvv_mode : THC_BVV_DEVICE; h->copy_stream = nullptr; h->copy_ready = false;
 
   // block sizes: defaults, then shrink until the plan fits the cap
@@ -633,13 +690,16 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
 
 int thc_destroy(thc_handle* h) {
   if (!h) return THC_ERR_INVALID_ARG;
-  if ((h->ws && h->ws_owned) || !h->prof_events.empty() || !h->tp_lists.empty() || h->copy_ready || h->sym_scratch) {
+  if ((h->ws && h->ws_owned) || !h->prof_events.empty() || !h->tp_lists.empty() || h->copy_ready || h->sym_scratch ||
+      h->cap_stream || h->graph[0].exec || h->graph[1].exec) {
     DeviceGuard g(h->device);
     cudaStreamSynchronize(h->stream);
     if (h->ws && h->ws_owned) cudaFree(h->ws);
     for (cudaEvent_t e : h->prof_events) cudaEventDestroy(e);
     for (auto& l : h->tp_lists) cudaFree(l.dev);
     if (h->sym_scratch) cudaFree(h->sym_scratch);
+    for (auto& gs : h->graph) if (gs.exec) cudaGraphExecDestroy(gs.exec);
+    if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
     if (h->copy_ready) {
       cudaStreamSynchronize(h->copy_stream);
       for (int k = 0; k < 2; k++) { cudaEventDestroy(h->ev_loaded[k]); cudaEventDestroy(h->ev_free[k]); }
@@ -697,13 +757,68 @@ int thc_residual_terms(thc_handle* h, const double* Xo, const double* Xv, const 
   int st = ensure_workspace(h, h->need_bytes);
   if (st != THC_OK) return st;
   if (h->check_symmetry && (st = check_symmetric(h, in, h->NL)) != THC_OK) return st;
-  return run_residual(h, static_cast<char*>(h->ws), h->ws_bytes, in, out);
+  std::vector<uintptr_t> key;
+  for (const void* q : {(const void*)Xo, (const void*)Xv, (const void*)Z, (const void*)B_ov, (const void*)B_oo, B_vv, (const void*)Y,
+                        (const void*)V, (const void*)eps, (const void*)R, (const void*)xi_oo, (const void*)xi_vv})
+    key.push_back(reinterpret_cast<uintptr_t>(q));
+  for (int k = 0; k < 6; k++) key.push_back(reinterpret_cast<uintptr_t>(out.terms[k]));
+  return run_maybe_graphed(h, 0, key, [&] { return run_residual(h, static_cast<char*>(h->ws), h->ws_bytes, in, out); });
 }
 
 int thc_residual(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov,
                  const double* B_oo, const void* B_vv, const double* Y, const double* V, const double* eps, double* R) {
   if (!R) return THC_ERR_INVALID_ARG;
   return thc_residual_terms(h, Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps, R, nullptr, nullptr, nullptr);
+}
+
+int64_t thc_workspace_bytes_rr(const thc_handle* h, int64_t NR) {
+  if (!h || NR <= 0) return (int64_t)THC_ERR_INVALID_ARG;
+  auto pad = [](i64 n) { return (n * 8 + 255) / 256 * 256; };
+  return h->need_bytes + 2 * pad(h->NP * h->NP) + pad(NR * h->NP) + 256;
+}
+
+int thc_residual_rr(thc_handle* h, int64_t NR, const double* tau, const double* T, const double* Xo, const double* Xv,
+                    const double* B_ov, const double* B_oo, const void* B_vv, const double* Y, const double* V,
+                    const double* eps, double* R_rr, double* Z_out) {
+  if (!h || NR <= 0 || NR >= ((int64_t)1 << 31)) return THC_ERR_INVALID_ARG;
+  if (bad_ptr(tau) || bad_ptr(T) || bad_ptr(Xo) || bad_ptr(Xv) || bad_ptr(B_ov) || bad_ptr(B_oo) || bad_ptr(B_vv) || bad_ptr(Y) ||
+      bad_ptr(V) || bad_ptr(eps) || bad_ptr(R_rr) || (Z_out && bad_ptr(Z_out)))
+    return THC_ERR_INVALID_ARG;
+  DeviceGuard g(h->device);
+  if (!g.ok) return THC_ERR_CUDA;
+  int st = ensure_workspace(h, thc_workspace_bytes_rr(h, NR));
+  if (st != THC_OK) return st;
+  const i64 NP = h->NP;
+  auto pad = [](i64 n) { return (n * 8 + 255) / 256 * 256; };
+  char* p = reinterpret_cast<char*>((reinterpret_cast<uintptr_t>(h->ws) + 255) / 256 * 256);
+  double* Z = reinterpret_cast<double*>(p); p += pad(NP * NP);
+  double* R = reinterpret_cast<double*>(p); p += pad(NP * NP);
+  double* tmp = reinterpret_cast<double*>(p); p += pad(NR * NP);
+  const i64 rest = h->ws_bytes - (p - static_cast<char*>(h->ws));
+  {
+    // Z[W][X] = sum_PQ tau[P][W] T[P][Q] tau[Q][X]:  tmp = T tau,  Z = tau^T tmp       (Eq.22 l.178)
+    Ctx c{h}; c.dry = false;
+    c.gemm(Gemm(T, NR, 'K', tau, NP, 'N', tmp, NP, NR, NP, NR));
+    c.gemm(Gemm(tau, NP, 'M', tmp, NP, 'N', Z, NP, NP, NP, NR));
+    if (c.status != THC_OK) return c.status;
+    if (Z_out) {
+      cudaError_t e = cudaMemcpyAsync(Z_out, Z, (size_t)NP * NP * 8, cudaMemcpyDeviceToDevice, h->stream);
+      if (e != cudaSuccess) { h->last_cuda = (int)e; return THC_ERR_CUDA; }
+    }
+  }
+  Inputs in{Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps};
+  Outputs out{};
+  out.R = R;
+  if (h->check_symmetry && (st = check_symmetric(h, in, h->NL)) != THC_OK) return st;
+  st = run_residual(h, p, rest, in, out);
+  if (st != THC_OK) return st;
+  {
+    // R_rr[P][Q] = sum_WX tau[P][W] R[W][X] tau[Q][X]:  tmp = tau R,  R_rr = tmp tau^T   (Eqs.6, 14)
+    Ctx c{h}; c.dry = false;
+    c.gemm(Gemm(tau, NP, 'K', R, NP, 'N', tmp, NP, NR, NP, NP));
+    c.gemm(Gemm(tmp, NP, 'K', tau, NP, 'K', R_rr, NR, NR, NR, NP));
+    return c.status;
+  }
 }
 
 int thc_energy(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* B_ov, double* E_host) {
@@ -721,7 +836,10 @@ int thc_energy_device(thc_handle* h, const double* Xo, const double* Xv, const d
   if (!g.ok) return THC_ERR_CUDA;
   int st = ensure_workspace(h, h->need_bytes);
   if (st != THC_OK) return st;
-  return run_energy(h, static_cast<char*>(h->ws), h->ws_bytes, Xo, Xv, Z, B_ov, nullptr, E_dev);
+  std::vector<uintptr_t> key;
+  for (const void* q : {(const void*)Xo, (const void*)Xv, (const void*)Z, (const void*)B_ov, (const void*)E_dev})
+    key.push_back(reinterpret_cast<uintptr_t>(q));
+  return run_maybe_graphed(h, 1, key, [&] { return run_energy(h, static_cast<char*>(h->ws), h->ws_bytes, Xo, Xv, Z, B_ov, nullptr, E_dev); });
 }
 
 // ---- sharded evaluation -----------------------------------------------------------------------------
@@ -953,17 +1071,16 @@ int thc_dgemm(thc_handle* h, int a_kmajor, int b_kmajor, int64_t M, int64_t N, i
 }
 
 int thc_triple_product(thc_handle* h, int64_t nI, int64_t nPp, int64_t NPp, const double* E, const double* F,
-                       const double* G, const double* GT, double* H, int accumulate) {
-  if (!h || bad_ptr(E) || bad_ptr(F) || bad_ptr(G) || bad_ptr(GT) || bad_ptr(H) || nI <= 0 || nPp <= 0 || NPp <= 0) return THC_ERR_INVALID_ARG;
+                       const double* G, double* H, int accumulate) {
+  if (!h || bad_ptr(E) || bad_ptr(F) || bad_ptr(G) || bad_ptr(H) || nI <= 0 || nPp <= 0 || NPp <= 0) return THC_ERR_INVALID_ARG;
   if (nPp % thc::TP_PT != 0 || NPp % thc::TP_RT != 0) return THC_ERR_INVALID_ARG;
-  if (((reinterpret_cast<uintptr_t>(E) | reinterpret_cast<uintptr_t>(F) | reinterpret_cast<uintptr_t>(G) | reinterpret_cast<uintptr_t>(GT) |
-        reinterpret_cast<uintptr_t>(H)) & 15) != 0)
+  if (((reinterpret_cast<uintptr_t>(E) | reinterpret_cast<uintptr_t>(F) | reinterpret_cast<uintptr_t>(G) | reinterpret_cast<uintptr_t>(H)) & 15) != 0)
     return THC_ERR_INVALID_ARG;
   DeviceGuard g(h->device);
   if (!g.ok) return THC_ERR_CUDA;
   Ctx c{h};
   c.dry = false;
-  c.triple_product(E, F, G, GT, H, nI, nPp, NPp, accumulate);
+  c.triple_product(E, F, G, H, nI, nPp, NPp, accumulate);
   return c.status;
 }
 

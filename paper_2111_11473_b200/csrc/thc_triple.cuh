@@ -17,9 +17,11 @@
 //     (TP_IC = 2 grid points, 4 KB per box) into a TP_STAGES-deep shared-memory ring; full/empty mbarriers, no
 //     __syncthreads in the I loop.  Thread 0 issues the boxes of stage j + TP_STAGES - 2 when it enters stage j (two
 //     stages of slack on the empty barrier; its counters live in shared memory), so ~120 KB are in flight per SM.  The
-//     mirrored block is read from a transposed copy of G (written by the GEMM epilogue) so that it has the same
-//     row-q / column-r access pattern as the direct one;
+//     mirrored block needs G_I[r][q]: it is read from the tile of G_I at (rows r-tile, columns q-tile) -- no transposed
+//     copy of G exists (it would double the memory of the I-chunk, which at paper scale decides the block sizes);
 //   * the 128-byte swizzle makes every 16-byte fragment load bank-conflict free (rows 4 apart differ in chunk bit 2);
+//     for the transposed reads of G the two halves of a quarter-warp would collide, so lanes with q bit 2 set read their
+//     row pairs in swapped order and swap the loaded values back with selects;
 //   * work items (p-tile, q-tile, r-tile) come from a host-built list ordered in groups of 8 p-tiles x 6 q-tiles x 3
 //     r-tiles, so that the ~148 CTAs running at the same time share their operand tiles in L2 (5x less HBM traffic).
 #pragma once
@@ -34,7 +36,7 @@ constexpr int TP_IC = 2;                                   // grid points per pi
 constexpr int TP_STAGES = 5, TP_LOOKAHEAD = TP_STAGES - 2;
 constexpr int TP_SLICE_BYTES = 16 * 16 * 8;                // one 16x16 FP64 block of one grid point
 constexpr int TP_BLK_BYTES = TP_IC * TP_SLICE_BYTES;       // one TMA box: 16 x 16 x TP_IC
-constexpr int TP_STAGE_BYTES = 10 * TP_BLK_BYTES;          // EPQ FPQ EPR0 EPR1 FPR0 FPR1 GQR0 GQR1 GTQR0 GTQR1
+constexpr int TP_STAGE_BYTES = 10 * TP_BLK_BYTES;          // EPQ FPQ EPR0 EPR1 FPR0 FPR1 GQR0 GQR1 GRQ0 GRQ1
 constexpr int TP_SMEM_BYTES = TP_STAGES * TP_STAGE_BYTES + 1024 /* alignment slack */ + 2 * TP_STAGES * 8;
 constexpr int TP_THREADS = 256;
 
@@ -82,16 +84,23 @@ __device__ __forceinline__ double2 lds128(const uint8_t* base, uint32_t off) {
 // sl + b * TP_BLK_BYTES).  hrq[a][b][c] accumulates H[p_a][r_c][q_b].
 template <bool DIAG>
 __device__ __forceinline__ void tp_update(const uint8_t* sl, const uint32_t (&offPQ)[4], const uint32_t (&offPR)[4],
-                                          const uint32_t (&offQR)[2], double (&hqr)[4][2][4], double (&hrq)[4][2][4]) {
-  double gqr[2][4], gt[2][4];            // gt[b][c] = G_I[r_c][q_b] (read from the transposed copy GT_I[q][r])
+                                          const uint32_t (&offQR)[2], uint32_t offT, bool swap, double (&hqr)[4][2][4],
+                                          double (&hrq)[4][2][4]) {
+  double gqr[2][4], gt[2][4];            // gt[b][c] = G_I[r_c][q_b], from the tile of G_I at (rows r, columns q)
 #pragma unroll
   for (int b = 0; b < 2; b++) {
     double2 g0 = lds128(sl, offQR[b]), g1 = lds128(sl, (offQR[b] ^ 64));
     gqr[b][0] = g0.x; gqr[b][1] = g0.y; gqr[b][2] = g1.x; gqr[b][3] = g1.y;
-    if (!DIAG) {
-      double2 h0 = lds128(sl, 2 * TP_BLK_BYTES + offQR[b]), h1 = lds128(sl, 2 * TP_BLK_BYTES + (offQR[b] ^ 64));
-      gt[b][0] = h0.x; gt[b][1] = h0.y; gt[b][2] = h1.x; gt[b][3] = h1.y;
-    }
+  }
+  if (!DIAG) {
+    // rows r_c = 2 lr + (c & 1) + 8 (c >> 1) of block 8 + wr; one 16-byte load gives (q_0, q_1) of a row.  offT is the
+    // offset of row 2 lr (+ 1 for `swap` lanes); the other row of the pair is at offT ^ 144 (next row, chunk bit 0
+    // flipped by the swizzle), rows + 8 are 1024 bytes further with the same swizzle phase.
+    const double2 t0 = lds128(sl, offT), t1 = lds128(sl, offT ^ 144), t2 = lds128(sl, offT + 1024), t3 = lds128(sl, (offT ^ 144) + 1024);
+    gt[0][0] = swap ? t1.x : t0.x; gt[1][0] = swap ? t1.y : t0.y;
+    gt[0][1] = swap ? t0.x : t1.x; gt[1][1] = swap ? t0.y : t1.y;
+    gt[0][2] = swap ? t3.x : t2.x; gt[1][2] = swap ? t3.y : t2.y;
+    gt[0][3] = swap ? t2.x : t3.x; gt[1][3] = swap ? t2.y : t3.y;
   }
 #pragma unroll
   for (int a = 0; a < 4; a++) {
@@ -111,13 +120,11 @@ __device__ __forceinline__ void tp_update(const uint8_t* sl, const uint32_t (&of
   }
 }
 
-// E, F: tensor maps over [nI][nPp][NPp] (innermost NPp); G, GT: over [nI][NPp][NPp] with GT_I[q][r] = G_I[r][q] (so that the
-// mirrored block is read with the same row-q / chunk-r pattern as the direct one); box 16 x 16 x TP_IC, SWIZZLE_128B.
+// E, F: tensor maps over [nI][nPp][NPp] (innermost NPp); G: over [nI][NPp][NPp]; box 16 x 16 x TP_IC, SWIZZLE_128B.
 // Grid points beyond nI (odd nI) are zero-filled by the TMA unit and add nothing.
 __global__ void __launch_bounds__(TP_THREADS, 1)
 triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_constant__ CUtensorMap mapF,
-                      const __grid_constant__ CUtensorMap mapG, const __grid_constant__ CUtensorMap mapGT,
-                      const TripleParams p) {
+                      const __grid_constant__ CUtensorMap mapG, const TripleParams p) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t ring = (smem_u32(smem_raw) + 1023u) & ~1023u;          // 1024-byte aligned (swizzle atom)
   const uint8_t* ring_ptr = smem_raw + (ring - smem_u32(smem_raw));
@@ -163,8 +170,8 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
     tma_load_3d(dst + 6 * TP_BLK_BYTES, &mapG, it.r0, it.q0, I, bf);
     tma_load_3d(dst + 7 * TP_BLK_BYTES, &mapG, it.r0 + 16, it.q0, I, bf);
     if (!it.diag) {
-      tma_load_3d(dst + 8 * TP_BLK_BYTES, &mapGT, it.r0, it.q0, I, bf);
-      tma_load_3d(dst + 9 * TP_BLK_BYTES, &mapGT, it.r0 + 16, it.q0, I, bf);
+      tma_load_3d(dst + 8 * TP_BLK_BYTES, &mapG, it.q0, it.r0, I, bf);          // rows r, columns q: the mirrored block
+      tma_load_3d(dst + 9 * TP_BLK_BYTES, &mapG, it.q0, it.r0 + 16, I, bf);
     }
     pj++;
     if (++pS == nS) { pS = 0; pk++; }
@@ -187,6 +194,9 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
     offQR[b] = (6 + wr) * TP_BLK_BYTES + row * 128 + ((lr ^ (row & 7)) << 4);
   }
 
+  const bool swap = (lane >> 2) & 1;                          // lanes whose q offset has bit 2 set (see tp_update)
+  const uint32_t offT = (((8 + wr) * TP_BLK_BYTES + (2 * lr) * 128 + ((cq ^ ((2 * lr) & 7)) << 4))) ^ (swap ? 144u : 0u);
+
   double hqr[4][2][4], hrq[4][2][4];
   int st = 0;                 // ring stage of the current iteration
   uint32_t par = 0;           // its mbarrier phase parity
@@ -206,10 +216,10 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
       const uint8_t* sl = ring_ptr + st * TP_STAGE_BYTES;
       if (diag) {
 #pragma unroll 1
-        for (int ii = 0; ii < TP_IC; ii++) tp_update<true>(sl + ii * TP_SLICE_BYTES, offPQ, offPR, offQR, hqr, hrq);
+        for (int ii = 0; ii < TP_IC; ii++) tp_update<true>(sl + ii * TP_SLICE_BYTES, offPQ, offPR, offQR, offT, swap, hqr, hrq);
       } else {
 #pragma unroll 1
-        for (int ii = 0; ii < TP_IC; ii++) tp_update<false>(sl + ii * TP_SLICE_BYTES, offPQ, offPR, offQR, hqr, hrq);
+        for (int ii = 0; ii < TP_IC; ii++) tp_update<false>(sl + ii * TP_SLICE_BYTES, offPQ, offPR, offQR, offT, swap, hqr, hrq);
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(bar_empty + 8 * st);

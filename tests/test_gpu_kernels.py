@@ -51,10 +51,9 @@ def test_triple_product_against_numpy(nI, nP, NPp):
     upd = np.einsum("ipq,ipr,iqr->pqr", E, F, G) + np.einsum("ipr,ipq,iqr->pqr", E, F, G)
     h = _handle()
     Ed, Fd, Gd = (torch.from_numpy(t).cuda() for t in (E, F, G))
-    GTd = torch.from_numpy(np.ascontiguousarray(G.transpose(0, 2, 1))).cuda()
     for acc in (0, 1):
         Hd = torch.from_numpy(H0).cuda()
-        h.thc_triple_product(nI, nP, NPp, Ed, Fd, Gd, GTd, Hd, acc)
+        h.thc_triple_product(nI, nP, NPp, Ed, Fd, Gd, Hd, acc)
         ref = upd + (H0 if acc else 0.0)
         got = Hd.cpu().numpy()
         assert np.abs(got - ref).max() <= 1e-13 * np.abs(ref).max() * max(1.0, np.sqrt(nI)), acc
