@@ -133,6 +133,23 @@ int thc_residual_terms(thc_handle* h, const double* Xo, const double* Xv, const 
                        const double* B_oo, const void* B_vv, const double* Y, const double* V,
                        const double* eps, double* R, double* const terms[6], double* xi_oo, double* xi_vv);
 
+/* T1-dressed evaluation: a complete CCSD residual.  With singles amplitudes t1[o][v] every Cholesky
+ * vector is dressed, B^ = Xp^T B Xh with Xp = 1 - t1 (occupied rows, virtual columns), Xh = 1 + t1^T (Eqs.25-27; in the
+ * MO basis the caller's B_oo, B_ov, B_vv are the BARE symmetric blocks, the library dresses them block by block and
+ * B^_vo != B^_ov^T), the Fock matrix becomes F^ = Xp^T h Xh + sum_k [2 (pq|kk)^ - (pk|kq)^] (h fixed by the bare Fock
+ * matrix being diag(eps)), and besides the doubles residual R_PQ (Eqs.28-41 with hatted integrals; the THC <ov|ov> terms
+ * are untouched because B^_ia = B_ia) the singles residual
+ *     sigma[o][v] = Omega G + Omega H (Eq.38 l.277; Alg.8 lines 11-12) + Omega I + Omega J (Eq.42 l.295; Alg.10)
+ * is returned (unprojected, as the paper's algorithms produce it).  The symmetric-product shortcuts of the half-transforms
+ * are switched off (only bra-ket symmetry is left, l.211); sigma1 stays symmetric.  terms[6] / sigma_terms[2] (G+H, I+J) /
+ * xi_oo / xi_vv are optional outputs (NULL allowed).  Needs thc_workspace_bytes_t1(h) bytes of workspace, all terms
+ * enabled (term_mask 0), and is evaluated on one device.  B_vv as in thc_residual. */
+int64_t thc_workspace_bytes_t1(const thc_handle* h);
+int thc_residual_t1(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* t1,
+                    const double* B_ov, const double* B_oo, const void* B_vv, const double* Y, const double* V,
+                    const double* eps, double* R, double* sigma, double* const terms[6], double* const sigma_terms[2],
+                    double* xi_oo, double* xi_vv);
+
 /* Rank-reduced working variables (Eqs.13-14 l.116-120, Eq.22 l.178-181): with the orthogonalised CP factor
  * tau[NR][NP] (tau~^{PW}, P < NR) and the symmetric core T[NR][NR] in the semi-unitary basis,
  *     Z = tau^T T tau                (the THC-basis core T^{WX} of Eq.22),

@@ -25,7 +25,7 @@ SYMBOLS = ("thc_setup", "thc_destroy", "thc_workspace_bytes", "thc_workspace_byt
            "thc_triple_product", "thc_strerror", "thc_last_cuda_error", "thc_last_error", "thc_shard_range",
            "thc_shard_doubles", "thc_residual_shard", "thc_residual_finish", "thc_energy_shard",
            "thc_profile_launches", "thc_profile_launch", "thc_algorithmic_work", "thc_probe", "thc_workspace_bytes_rr",
-           "thc_residual_rr")
+           "thc_residual_rr", "thc_workspace_bytes_t1", "thc_residual_t1")
 
 TERM_NAMES = ("s1", "s2", "s3", "s6", "s7", "s9")
 TERM_BITS = dict(s1=1, s2=2, s3=4, s6=8, s7=16, s9=32)
@@ -114,6 +114,9 @@ def lib() -> ctypes.CDLL:
     L.thc_workspace_bytes_rr.argtypes = [VP, I64]
     L.thc_workspace_bytes_rr.restype = I64
     L.thc_residual_rr.argtypes = [VP, I64] + [P] * 12
+    L.thc_workspace_bytes_t1.argtypes = [VP]
+    L.thc_workspace_bytes_t1.restype = I64
+    L.thc_residual_t1.argtypes = [VP] + [P] * 12 + [ctypes.POINTER(P * 6), ctypes.POINTER(P * 2), P, P]
     L.thc_residual_host.argtypes = [VP] + [P] * 10 + [ctypes.POINTER(D)]
     L.thc_kernel_launches.argtypes = [VP]
     L.thc_kernel_launches.restype = I64
@@ -275,6 +278,23 @@ class Thc:
         ptrs = self._in_ptrs(Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps, _dev_ptr)
         _check(lib().thc_residual_terms(self._h, *ptrs, _dev_ptr(res["R"], "R"), ctypes.byref(terms),
                                         _dev_ptr(res["xi_oo"], "xi_oo"), _dev_ptr(res["xi_vv"], "xi_vv")), self._h)
+        return res
+
+    def thc_residual_t1(self, Xo, Xv, Z, t1, B_ov, B_oo, B_vv, Y, V, eps):
+        """T1-dressed evaluation: dict with R, s1..s9 [NP, NP], sigma, sigma_GH, sigma_IJ [o, v], xi_oo, xi_vv."""
+        import torch
+        self._prepare(max(self.workspace_bytes, int(lib().thc_workspace_bytes_t1(self._h))))
+        kw = dict(dtype=torch.float64, device=self._device)
+        res = {k: torch.empty(self.NP, self.NP, **kw) for k in ("R",) + TERM_NAMES}
+        for k in ("sigma", "sigma_GH", "sigma_IJ"):
+            res[k] = torch.empty(self.o, self.v, **kw)
+        res["xi_oo"], res["xi_vv"] = torch.empty(self.o, self.o, **kw), torch.empty(self.v, self.v, **kw)
+        terms = (ctypes.c_void_p * 6)(*[res[k].data_ptr() for k in TERM_NAMES])
+        parts = (ctypes.c_void_p * 2)(res["sigma_GH"].data_ptr(), res["sigma_IJ"].data_ptr())
+        p = self._in_ptrs(Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps, _dev_ptr)
+        _check(lib().thc_residual_t1(self._h, p[0], p[1], p[2], _dev_ptr(t1, "t1", self.o * self.v), p[3], p[4], p[5], p[6],
+                                     p[7], p[8], _dev_ptr(res["R"], "R"), _dev_ptr(res["sigma"], "sigma"), ctypes.byref(terms),
+                                     ctypes.byref(parts), _dev_ptr(res["xi_oo"], "xi_oo"), _dev_ptr(res["xi_vv"], "xi_vv")), self._h)
         return res
 
     def thc_residual_rr(self, tau, T, Xo, Xv, B_ov, B_oo, B_vv, Y, V, eps, want_Z=False):

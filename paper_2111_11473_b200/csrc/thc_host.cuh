@@ -448,6 +448,12 @@ struct Ctx {
     launched();
     prof_stop(2);
   }
+  void t1_eps(const double* eps, const double* t1, double* out, i64 o, i64 v) { THC_EW(t1_eps_kernel, o * v, 24.0 * o * v, eps, t1, out, (int)o, (int)v); }
+  void diag(const double* A, double* d, i64 n) { THC_EW(diag_kernel, n, 16.0 * n, A, d, (int)n); }
+  void copy(const double* src, double* dst, i64 n) {
+    if (dry || !ok()) return;
+    check(cudaMemcpyAsync(dst, src, (size_t)n * 8, cudaMemcpyDeviceToDevice, h->stream));
+  }
   void fock(const double* eps, const double* xi_oo, const double* xi_vv, double* FooT, double* Fvv, i64 o, i64 v) {
     THC_EW(fock_kernel, o * o + v * v, 16.0 * (o * o + v * v), eps, xi_oo, xi_vv, FooT, Fvv, (int)o, (int)v);
   }

@@ -32,13 +32,12 @@ __global__ void fill_kernel(double* __restrict__ x, i64 n, double val) {
 }
 
 // out = a .* b                                   (w = o .* v, Alg.3 l.596, Alg.7 l.736, Alg.9 l.817)
-__global__ void hadamard_kernel(const double* __restrict__ a, const double* __restrict__ b, double* __restrict__ out, i64 n) {
+__global__ void hadamard_kernel(const double* a, const double* b, double* out, i64 n) {      // out may alias a or b
   THC_GRID_STRIDE(i, n) out[i] = a[i] * b[i];
 }
 
 // out = ca * a + cb * b
-__global__ void axpby_kernel(const double* __restrict__ a, const double* __restrict__ b, double ca, double cb,
-                             double* __restrict__ out, i64 n) {
+__global__ void axpby_kernel(const double* a, const double* b, double ca, double cb, double* out, i64 n) {   // out may alias a or b
   THC_GRID_STRIDE(i, n) out[i] = ca * a[i] + cb * b[i];
 }
 
@@ -61,6 +60,19 @@ __global__ void combine_kernel(double* __restrict__ Mo, const double* __restrict
     }
     C3[i] += c3;
   }
+}
+
+// FvoT[i][a] = (eps[o+a] - eps[i]) * t1[i][a]: the one-electron part of the dressed Fock matrix F^_ai (canonical orbitals)
+__global__ void t1_eps_kernel(const double* __restrict__ eps, const double* __restrict__ t1, double* __restrict__ out, int o, int v) {
+  THC_GRID_STRIDE(idx, (i64)o * v) {
+    const int i = (int)(idx / v), a = (int)(idx % v);
+    out[idx] = (eps[o + a] - eps[i]) * t1[idx];
+  }
+}
+
+// d[P] = A[P][P]
+__global__ void diag_kernel(const double* __restrict__ A, double* __restrict__ d, int n) {
+  THC_GRID_STRIDE(idx, (i64)n) d[idx] = A[idx * n + idx];
 }
 
 // out[b*ldo + r] = sum_{i<n} X[r*ldx + i] * T[b*sTb + r*ldT + i]      (a^L_P: Alg.2 l.541, Alg.8 l.788; C7: Alg.7 line 9 l.749)

@@ -25,12 +25,15 @@ struct Inputs {
   const double *Xo, *Xv, *Z, *B_ov, *B_oo;
   const void* B_vv;        // device array, host array or thc_bvv_provider*, per thc_options.bvv_mode (thc.h)
   const double *Y, *V, *eps;
+  const double* t1 = nullptr;    // [o][v] singles amplitudes: T1-dressed evaluation, else NULL
 };
 struct Outputs {
   double* R;
   double* terms[6];   // s1 s2 s3 s6 s7 s9 (NULL -> scratch)
   double* xi_oo;
   double* xi_vv;
+  double* sigma = nullptr;                         // [o][v] singles residual (T1 evaluation only)
+  double* sigma_parts[2] = {nullptr, nullptr};     // Omega G+H (Eq.38), Omega I+J (Eq.42)
 };
 // Sharded evaluation: phase 1 computes one rank's partial
 // sums over its Cholesky range [Lb, Le) and its rows [Pb, Pe) of the T2^2 terms into `packed`; after the caller has
@@ -87,6 +90,18 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out, const Shard& sh
   double* C3 = sh.phase ? sh.packed + pk.C3 : ar.alloc(NP2);
   double *Aa = ar.alloc(std::max<i64>(NL, 1) * NP), *Dm = ar.alloc(std::max<i64>(NL, 1) * NP);
 
+  // T1-dressed evaluation (phase 0 only): accumulators of the dressed Fock matrix minus diag(eps), in the layouts the
+  // later steps read (Fd_oo[i][j] = F^_ij, FdT_vv[b][a] = F^_ab, F_ov[i][a], F_voT[i][a] = F^_ai), and of the singles
+  // residual.  F^_pq = (Xp^T diag(eps) Xh)_pq + sum_L [ 2 B^_pq tau^L - sum_kc (pc|kq)^-like exchange ], tau^L = sum_kc B_kc t_k^c.
+  const double* t1 = sh.phase == 0 ? in.t1 : nullptr;
+  double *Fd_oo = nullptr, *FdT_vv = nullptr, *F_ov = nullptr, *F_voT = nullptr, *sigGH = nullptr, *sigIJ = nullptr, *Abar = nullptr;
+  if (t1) {
+    Fd_oo = ar.alloc(o * o); FdT_vv = ar.alloc(v * v); F_ov = ar.alloc(ov); F_voT = ar.alloc(ov);
+    sigGH = out.sigma_parts[0] ? out.sigma_parts[0] : ar.alloc(ov);
+    sigIJ = out.sigma_parts[1] ? out.sigma_parts[1] : ar.alloc(ov);
+    Abar = ar.alloc(std::max<i64>(NL, 1) * NP);
+  }
+
   // ---- H0: transposed factors and grams (Alg.1 l.481-485) ------------------------------------------------------------
   c.transpose(in.Xo, XoT, o, NP);
   c.transpose(in.Xv, XvT, v, NP);
@@ -102,13 +117,18 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out, const Shard& sh
     c.fill(s1, NP2, 0.0);
     c.fill(xi_oo, o * o, 0.0);
     c.fill(xi_vv, v * v, 0.0);
+    if (t1) {
+      c.fill(Fd_oo, o * o, 0.0); c.fill(FdT_vv, v * v, 0.0); c.fill(F_ov, ov, 0.0); c.fill(sigGH, ov, 0.0);
+      c.t1_eps(in.eps, t1, F_voT, o, v);                 // (eps_a - eps_i) t_i^a: Xp^T diag(eps) Xh, vo block
+    }
   }
 
   // ---- L-block loop: Alg.1 + Alg.3 (H1-H4) and Alg.2 + Alg.8 (H5-H6) fused over the Cholesky index (l.238) ---------
   const bool need_ladder = local && (do_s1 || do_s3);
-  const bool need_ring = local && (do_s2 || do_s9);
+  const bool need_ring = local && (do_s2 || do_s9 || t1);
+  const bool need_bvv = need_ladder || t1;       // the dressed vv blocks also feed the singles residual and F^
   // B_vv source: resident (device pointer), or streamed one L-block at a time into a double buffer (l.191-195)
-  const bool streamed = h->bvv_mode != THC_BVV_DEVICE && need_ladder;
+  const bool streamed = h->bvv_mode != THC_BVV_DEVICE && need_bvv;
   double* bvv_buf[2] = {nullptr, nullptr};
   if (streamed) { bvv_buf[0] = ar.alloc(h->bL * v * v); bvv_buf[1] = ar.alloc(h->bL * v * v); }
   if (streamed && !c.dry) c.bvv_begin();
@@ -117,7 +137,7 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out, const Shard& sh
   i64 blk = 0;
   for (i64 L0 = 0; L0 < NL; L0 += h->bL, blk++) {
     const i64 nl = std::min<i64>(h->bL, NL - L0);
-    const i64 m0 = ar.mark();
+    const i64 mT = ar.mark();
     const double* bvv = static_cast<const double*>(in.B_vv) + L0 * v * v;
     if (streamed) {
       bvv = bvv_buf[blk & 1];
@@ -131,20 +151,59 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out, const Shard& sh
         }
       }
     }
+    // ---- T1 dressing of this block (Eqs.25-27 l.203-209 in the MO basis).  Index order matters now (l.211).  Projecting
+    // Eq.28 term by term gives C^L = v .* Bbar^T - o .* Btilde with Bbar^{XY} = sum_ki y_k^X l_ki y_i^Y and
+    // Btilde^{XY} = sum_ac y_a^X l_ac y_c^Y (at t1 = 0 the transpose is invisible; Alg.1 lines 6-8 as printed pair X with
+    // the first index of l_ki, which the determinant-space pin of oracle/t1.py rules out), and Eq.38 gives
+    // -sum_k l_ki D_ka for Alg.8 line 12.  The half-transforms below contract the SECOND index of a stored block first,
+    // so the dressed oo block is kept in natural order (Boo_h[l][k][j] = B^_kj -> Mo = Bbar^T) and the dressed vv block
+    // transposed (BvvT[l][c][a] = B^_ac -> Mv = Btilde).
+    const double* boo = in.B_oo + L0 * o * o;
+    const double* bov = in.B_ov + L0 * ov;
+    double *TL = nullptr, *Boo_h = nullptr, *BvvT = nullptr, *BvoT = nullptr, *Sl = nullptr, *tau = nullptr;
+    if (t1) {
+      TL = ar.alloc(nl * o * o); Boo_h = ar.alloc(nl * o * o); BvoT = ar.alloc(nl * ov); Sl = ar.alloc(nl * v * o); tau = ar.alloc(nl);
+      BvvT = streamed ? bvv_buf[blk & 1] : ar.alloc(nl * v * v);       // a streamed block is ours: dress it in place
+      // TL[l][k][j] = sum_a B_ka t_j^a ;  B^_kj = B_kj + TL[l][k][j]
+      c.gemm(Gemm(bov, v, 'K', t1, v, 'K', TL, o, nl * o, o, v));
+      c.axpby(boo, TL, 1.0, 1.0, Boo_h, nl * o * o);
+      // B^_ac = B_ac - sum_i t_i^a B_ic, stored as BvvT[l][c][a]
+      if (!streamed) c.copy(bvv, BvvT, nl * v * v);
+      c.gemm(Gemm(bov, v, 'M', t1, v, 'N', BvvT, v, v, v, o).batch(nl, ov, 0, v * v).ab(-1.0, 1.0));
+      // tau^l = sum_kc B_kc t_k^c ;  Sl[l][a][k] = sum_c B^_ac t_k^c
+      c.rowdot(t1, ov, bov, ov, ov, tau, 1, nl, 1, ov);
+      c.gemm(Gemm(BvvT, v, 'M', t1, v, 'K', Sl, o, v, o, v).batch(nl, v * v, 0, v * o));
+      // B^_ai = B_ia - sum_j t_j^a B_ji + sum_b B^_ab t_i^b, stored as BvoT[l][i][a]
+      c.copy(bov, BvoT, nl * ov);
+      c.gemm(Gemm(boo, o, 'K', t1, v, 'N', BvoT, v, o, v, o).batch(nl, o * o, 0, ov).ab(-1.0, 1.0));
+      c.gemm(Gemm(t1, v, 'K', BvvT, v, 'N', BvoT, v, o, v, v).batch(nl, 0, v * v, ov).ab(1.0, 1.0));
+      // dressed Fock matrix: 2 tau^l B^ parts (one GEMV-shaped product over l each) and the exchange parts
+      c.gemm(Gemm(tau, nl, 'K', Boo_h, o * o, 'N', Fd_oo, o * o, 1, o * o, nl).ab(2.0, 1.0));
+      c.gemm(Gemm(TL, o, 'K', Boo_h, o, 'N', Fd_oo, o, o, o, o).kbatch(nl, o * o, o * o).ab(-1.0, 1.0));       // sum_k T[i][k] B^_kj
+      c.gemm(Gemm(tau, nl, 'K', BvvT, v * v, 'N', FdT_vv, v * v, 1, v * v, nl).ab(2.0, 1.0));
+      c.gemm(Gemm(bov, v, 'M', Sl, o, 'K', FdT_vv, v, v, v, o).kbatch(nl, ov, v * o).ab(-1.0, 1.0));         // sum_k B_kb S[a][k]
+      c.gemm(Gemm(tau, nl, 'K', bov, ov, 'N', F_ov, ov, 1, ov, nl).ab(2.0, 1.0));
+      c.gemm(Gemm(TL, o, 'K', bov, v, 'N', F_ov, v, o, v, o).kbatch(nl, o * o, ov).ab(-1.0, 1.0));            // sum_k T[i][k] B_ka
+      c.gemm(Gemm(tau, nl, 'K', BvoT, ov, 'N', F_voT, ov, 1, ov, nl).ab(2.0, 1.0));
+      c.gemm(Gemm(Boo_h, o, 'M', Sl, o, 'K', F_voT, v, o, v, o).kbatch(nl, o * o, v * o).ab(-1.0, 1.0));      // sum_k B^_ki S[a][k]
+      boo = Boo_h;
+      bvv = BvvT;
+    }
+    const i64 m0 = ar.mark();
     if (need_ladder) {
       double* T1T = ar.alloc(NP * nl * o);
       double* T2T = ar.alloc(NP * nl * v);
       double *Mo = ar.alloc(nl * NP2), *Mv = ar.alloc(nl * NP2);
       // H1: T1T[P][(l,j)] = sum_i Xo[i,P] B^l_ij ;  Mo^l[P][Q] = sum_j T1T[P][(l,j)] Xo[j,Q]      (Alg.1 lines 6-7)
-      c.gemm(Gemm(XoT, o, 'K', in.B_oo + L0 * o * o, o, 'K', T1T, nl * o, NP, nl * o, o));
+      c.gemm(Gemm(XoT, o, 'K', boo, o, 'K', T1T, nl * o, NP, nl * o, o));
       // (B^l symmetric => M^{o,l}, M^{v,l} symmetric: for NP of several tiles only the upper tiles are computed and the
       //  lower ones mirrored in one batched pass; for small NP the mirror pass costs more than it saves)
-      const bool sym_half = NP >= 640;
+      const bool sym_half = NP >= 640 && !t1;          // dressed vectors are not symmetric (l.211)
       Gemm gMo = Gemm(T1T, nl * o, 'K', XoT, o, 'K', Mo, NP, NP, NP, o).batch(nl, o, 0, NP2);
       c.gemm(sym_half ? gMo.upper_only() : gMo);
       // H2: same with the vv block                                                                  (Alg.1 lines 10-11)
       c.gemm(Gemm(XvT, v, 'K', bvv, v, 'K', T2T, nl * v, NP, nl * v, v));
-      if (streamed && !c.dry && h->bvv_mode == THC_BVV_HOST) c.bvv_release(blk);
+      if (streamed && !c.dry && h->bvv_mode == THC_BVV_HOST && !t1) c.bvv_release(blk);
       Gemm gMv = Gemm(T2T, nl * v, 'K', XvT, v, 'K', Mv, NP, NP, NP, v).batch(nl, v, 0, NP2);
       c.gemm(sym_half ? gMv.upper_only() : gMv);
       if (sym_half) { c.mirror_upper(Mo, NP, nl); c.mirror_upper(Mv, NP, nl); }
@@ -182,8 +241,18 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out, const Shard& sh
       double* DX = ar.alloc(nl * o * NP);
       c.gemm(Gemm(Dia, v, 'K', XvT, v, 'K', DX, NP, nl * o, NP, v));
       c.coldot(in.Xo, NP, DX, o * NP, NP, Dm + L0 * NP, NP, nl, NP, o);
+      if (t1) {
+        // A-bar^l_P = sum_ia Xo[i,P] Xv[a,P] B^_ai                                                       (Eq.30 l.229; Alg.2 line 4)
+        c.gemm(Gemm(XvT, v, 'K', BvoT, v, 'K', TT, nl * o, NP, nl * o, v));
+        c.rowdot(XoT, o, TT, o, nl * o, Abar + L0 * NP, NP, nl, NP, o);
+        // Omega G, H: sigma_ia += sum_b D^l_ib B^_ab - sum_k B^_ki D^l_ka                                (Alg.8 lines 11-12 l.800-803; Eq.38)
+        c.gemm(Gemm(Dia, v, 'K', BvvT, v, 'N', sigGH, v, o, v, v).kbatch(nl, ov, v * v).ab(1.0, 1.0));
+        c.gemm(Gemm(Boo_h, o, 'M', Dia, v, 'N', sigGH, v, o, v, o).kbatch(nl, o * o, ov).ab(-1.0, 1.0));         // sum_k B^_ki D_ka
+      }
       ar.release(m0);
     }
+    if (streamed && !c.dry && h->bvv_mode == THC_BVV_HOST && t1) c.bvv_release(blk);     // the dressed block was read until here
+    ar.release(mT);
   }
 
   if (local && do_s1) c.mirror_upper(s1, NP);          // complete the symmetric sigma1 from its upper triangle
@@ -193,10 +262,12 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out, const Shard& sh
     // phase 2: s2 arrives summed over the ranks
   } else if (do_s2 && NL > 0) {
     const i64 m0 = ar.mark();
+    // (T1: the bare term and the partners of D use A-bar from the dressed vo block, Alg.2 line 14 l.559; Dm comes from l_ia)
+    const double* A2 = t1 ? Abar : Aa;
     double* AD = ar.alloc(NL * NP);
-    c.axpby(Aa, Dm, 1.0, 1.0, AD, NL * NP);
-    c.gemm(Gemm(AD, NP, 'M', Aa, NP, 'N', s2, NP, NP, NP, NL));
-    c.gemm(Gemm(Aa, NP, 'M', Dm, NP, 'N', s2, NP, NP, NP, NL).ab(1.0, 1.0));
+    c.axpby(A2, Dm, 1.0, 1.0, AD, NL * NP);
+    c.gemm(Gemm(AD, NP, 'M', A2, NP, 'N', s2, NP, NP, NP, NL));
+    c.gemm(Gemm(A2, NP, 'M', Dm, NP, 'N', s2, NP, NP, NP, NL).ab(1.0, 1.0));
     ar.release(m0);
   } else {
     c.fill(s2, NP2, 0.0);
@@ -222,7 +293,15 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out, const Shard& sh
     double *FooT = ar.alloc(o * o), *Fvv = ar.alloc(v * v);
     double *CoT = ar.alloc(NP * o), *DvT = ar.alloc(NP * v), *otil = ar.alloc(NP2), *vtil = ar.alloc(NP2);
     double *E9 = ar.alloc(NP2), *P9 = ar.alloc(NP2);
-    c.fock(in.eps, xi_oo, xi_vv, FooT, Fvv, o, v);
+    if (t1) {                                   // F' = F^ + xi: add the dressing parts to copies of xi before the diagonal
+      double *Xoo = ar.alloc(o * o), *Xvv = ar.alloc(v * v);
+      c.axpby(xi_oo, Fd_oo, 1.0, 1.0, Xoo, o * o);
+      c.transpose(FdT_vv, Xvv, v, v);
+      c.axpby(Xvv, xi_vv, 1.0, 1.0, Xvv, v * v);
+      c.fock(in.eps, Xoo, Xvv, FooT, Fvv, o, v);
+    } else {
+      c.fock(in.eps, xi_oo, xi_vv, FooT, Fvv, o, v);
+    }
     c.gemm(Gemm(XoT, o, 'K', FooT, o, 'K', CoT, o, NP, o, o));         // CoT[P][i] = sum_j Xo[j,P] F'[j][i]
     c.gemm(Gemm(XoT, o, 'K', CoT, o, 'K', otil, NP, NP, NP, o));       // o~[P][Q] = sum_i Xo[i,P] C_i^Q
     c.gemm(Gemm(XvT, v, 'K', Fvv, v, 'K', DvT, v, NP, v, v));          // DvT[P][a] = sum_b Xv[b,P] F'[a][b]
@@ -351,6 +430,24 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out, const Shard& sh
     c.fill(s6, NP2, 0.0);
   }
 
+  // ---- Omega I, J: sigma_ia = F^_ai + sum_kc (2 t_ik^ac - t_ik^ca) F^_kc   (Eq.42 l.295; Alg.10 l.845-876) ----------------
+  if (t1) {
+    const i64 m0 = ar.mark();
+    double *AX = ar.alloc(o * NP), *BB = ar.alloc(NP2), *dB = ar.alloc(NP), *Cx = ar.alloc(NP), *FX = ar.alloc(o * NP), *G = ar.alloc(o * NP);
+    c.gemm(Gemm(F_ov, v, 'K', XvT, v, 'K', AX, NP, o, NP, v));                   // line 1: A_i^X = sum_a F^_ia y_a^X
+    c.gemm(Gemm(XoT, o, 'K', AX, NP, 'N', BB, NP, NP, NP, o));                   // line 2: B^{XY} = sum_i y_i^X A_i^Y
+    c.diag(BB, dB, NP);
+    c.gemm(Gemm(dB, NP, 'K', in.Z, NP, 'K', Cx, NP, 1, NP, NP));                 // line 3: C^X = sum_Y T^{XY} B^{YY}
+    c.hadamard(in.Z, BB, BB, NP2);                                               // line 6: E = T .* B
+    c.gemm(Gemm(in.Xo, NP, 'K', BB, NP, 'K', FX, NP, o, NP, NP));                // line 7: F_i^X = sum_Y y_i^Y E^{XY}
+    c.rowscale(in.Xo, NP, Cx, NP, nullptr, 2.0, G, 1, o, NP);                    // lines 4-5, 8: (2 y_i^X C^X - F_i^X) y_a^X
+    c.axpby(G, FX, 1.0, -1.0, G, o * NP);
+    c.copy(F_voT, sigIJ, ov);                                                    // line 10: + F^_ai
+    c.gemm(Gemm(G, NP, 'K', in.Xv, NP, 'K', sigIJ, v, o, v, NP).ab(1.0, 1.0));
+    if (out.sigma) c.axpby(sigGH, sigIJ, 1.0, 1.0, out.sigma, ov);
+    ar.release(m0);
+  }
+
   // ---- H11 ---------------------------------------------------------------------------------------------------------
   if (out.R) c.sum6(term, out.R, NP2);
 }
@@ -391,9 +488,10 @@ void plan_energy(Ctx& c, const double* Xo, const double* Xv, const double* Z, co
 // ---- dry runs: workspace sizes for the three entry points ------------------------------------------------------------
 struct Need { i64 arena_bytes, splitk_doubles; i64 total() const { return arena_bytes + (splitk_doubles * 8 + 255) / 256 * 256 + 256; } };
 
-Need dry_residual(thc_handle* h) {
+Need dry_residual(thc_handle* h, bool with_t1 = false) {
   Ctx c{h}; c.dry = true; c.ar.dry = true;
   Inputs in{}; Outputs out{};
+  if (with_t1) in.t1 = reinterpret_cast<const double*>(static_cast<uintptr_t>(256));     // only its non-nullness is used
   plan_residual(c, in, out);
   return Need{c.ar.peak, c.splitk_need};
 }
@@ -488,7 +586,7 @@ struct DeviceGuard {
 };
 
 int run_residual(thc_handle* h, char* base, i64 bytes, const Inputs& in, const Outputs& out, const Shard& sh = Shard()) {
-  Need need = dry_residual(h);
+  Need need = dry_residual(h, in.t1 != nullptr && sh.phase == 0);
   Ctx c{h};
   int st = make_ctx(c, h, base, bytes, need);
   if (st != THC_OK) return st;
@@ -646,12 +744,12 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
     h->bX = sX; h->bI = sI;
     if (!fix_bX && !fix_bI && need_device(h) > cap) {
       const double fo = (double)o, fv = (double)v, fNP = (double)NP, fNX = (double)NX;
-      // measured on B200 (profiles/): the K = NX and K = v products of a G pass run at ~30 TFLOP/s, the K = o product
-      // with its N x N output at ~22; the read-modify-write of H at the end of every work item of line 11 is not
-      // overlapped with its FMAs, so it costs about twice its HBM time.  (+ A3 rebuilt per row block when not resident.)
-      const double t_g = fNX * ((2 * fo * fv * fNX + 2 * fo * fv * fNP) / 30e12 + 2 * fo * fNP * fNP / 22e12) +
-                         (NP * o * v * 8 > ((i64)4 << 30) ? 2 * fNP * fNP * fo * fv / 30e12 : 0.0);           // DMMA, s
-      const double t_h = 16.0 * fNP * (double)pad_to(NP, 32) * (double)pad_to(NP, 32) / 2.5e12;          // HBM, s
+      // measured on B200 (profiles/r02_final.md, config 4): one G pass (B_ia^I, its two half-transforms, A3 rebuilt when it
+      // is not resident) runs at ~30 TFLOP/s = 9.6 s; the read-modify-write of H at the end of every work item of line 11
+      // is not overlapped with its FMAs and costs its HBM time at ~4 TB/s.
+      const double t_g = (fNX * (2 * fo * fv * fNX + 2 * fo * fv * fNP + 2 * fo * fNP * fNP) +
+                          (NP * o * v * 8 > ((i64)4 << 30) ? 2 * fNP * fNP * fo * fv : 0.0)) / 30e12;            // DMMA, s
+      const double t_h = 16.0 * fNP * (double)pad_to(NP, 32) * (double)pad_to(NP, 32) / 4e12;            // HBM, s
       double best = 1e300; int64_t bestX = 0, bestI = 0;
       // (chunks of a multiple of 128 grid points fill the 128-row tiles of the E_I / F_I products)
       for (int64_t bi : {16, 32, 64, 128, 256, 384, 512, 640, 768, 896, 1024}) {
@@ -769,6 +867,32 @@ int thc_residual(thc_handle* h, const double* Xo, const double* Xv, const double
                  const double* B_oo, const void* B_vv, const double* Y, const double* V, const double* eps, double* R) {
   if (!R) return THC_ERR_INVALID_ARG;
   return thc_residual_terms(h, Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps, R, nullptr, nullptr, nullptr);
+}
+
+int64_t thc_workspace_bytes_t1(const thc_handle* h) {
+  return h ? dry_residual(const_cast<thc_handle*>(h), true).total() : (int64_t)THC_ERR_INVALID_ARG;
+}
+
+int thc_residual_t1(thc_handle* h, const double* Xo, const double* Xv, const double* Z, const double* t1, const double* B_ov,
+                    const double* B_oo, const void* B_vv, const double* Y, const double* V, const double* eps, double* R,
+                    double* sigma, double* const terms[6], double* const sigma_terms[2], double* xi_oo, double* xi_vv) {
+  if (!h) return THC_ERR_INVALID_ARG;
+  if (bad_ptr(Xo) || bad_ptr(Xv) || bad_ptr(Z) || bad_ptr(t1) || bad_ptr(B_ov) || bad_ptr(B_oo) || bad_ptr(B_vv) || bad_ptr(Y) ||
+      bad_ptr(V) || bad_ptr(eps) || bad_ptr(R) || bad_ptr(sigma) || (xi_oo && bad_ptr(xi_oo)) || (xi_vv && bad_ptr(xi_vv)))
+    return THC_ERR_INVALID_ARG;
+  if ((h->term_mask ? h->term_mask : THC_TERM_ALL) != THC_TERM_ALL) return THC_ERR_INVALID_ARG;     // a complete residual only
+  Inputs in{Xo, Xv, Z, B_ov, B_oo, B_vv, Y, V, eps};
+  in.t1 = t1;
+  Outputs out{};
+  out.R = R; out.sigma = sigma; out.xi_oo = xi_oo; out.xi_vv = xi_vv;
+  for (int k = 0; k < 6; k++) out.terms[k] = terms ? terms[k] : nullptr;
+  for (int k = 0; k < 2; k++) out.sigma_parts[k] = sigma_terms ? sigma_terms[k] : nullptr;
+  DeviceGuard g(h->device);
+  if (!g.ok) return THC_ERR_CUDA;
+  int st = ensure_workspace(h, std::max<i64>(h->need_bytes, thc_workspace_bytes_t1(h)));
+  if (st != THC_OK) return st;
+  if (h->check_symmetry && (st = check_symmetric(h, in, h->NL)) != THC_OK) return st;
+  return run_residual(h, static_cast<char*>(h->ws), h->ws_bytes, in, out);
 }
 
 int64_t thc_workspace_bytes_rr(const thc_handle* h, int64_t NR) {

@@ -19,9 +19,10 @@
 //     stages of slack on the empty barrier; its counters live in shared memory), so ~120 KB are in flight per SM.  The
 //     mirrored block needs G_I[r][q]: it is read from the tile of G_I at (rows r-tile, columns q-tile) -- no transposed
 //     copy of G exists (it would double the memory of the I-chunk, which at paper scale decides the block sizes);
-//   * the 128-byte swizzle makes every 16-byte fragment load bank-conflict free (rows 4 apart differ in chunk bit 2);
-//     for the transposed reads of G the two halves of a quarter-warp would collide, so lanes with q bit 2 set read their
-//     row pairs in swapped order and swap the loaded values back with selects;
+//   * the 128-byte swizzle makes every 16-byte fragment load bank-conflict free.  The eight lanes of a quarter-warp are
+//     four r offsets x two q offsets; the two q offsets are chosen 6 or 2 apart (q pairs 0/3 and 1/2 of the warp's four),
+//     so that they differ both in bit 2 of the row (direct reads of G: rows q, chunks r) and in bit 0 of the 16-byte
+//     chunk (transposed reads of G: rows r, chunks q) -- both read patterns hit eight different chunks;
 //   * work items (p-tile, q-tile, r-tile) come from a host-built list ordered in groups of 8 p-tiles x 6 q-tiles x 3
 //     r-tiles, so that the ~148 CTAs running at the same time share their operand tiles in L2 (5x less HBM traffic).
 #pragma once
@@ -75,6 +76,7 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map
       "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
       ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
 }
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 __device__ __forceinline__ double2 lds128(const uint8_t* base, uint32_t off) {
   return *reinterpret_cast<const double2*>(base + off);
 }
@@ -84,7 +86,7 @@ __device__ __forceinline__ double2 lds128(const uint8_t* base, uint32_t off) {
 // sl + b * TP_BLK_BYTES).  hrq[a][b][c] accumulates H[p_a][r_c][q_b].
 template <bool DIAG>
 __device__ __forceinline__ void tp_update(const uint8_t* sl, const uint32_t (&offPQ)[4], const uint32_t (&offPR)[4],
-                                          const uint32_t (&offQR)[2], uint32_t offT, bool swap, double (&hqr)[4][2][4],
+                                          const uint32_t (&offQR)[2], uint32_t offT, double (&hqr)[4][2][4],
                                           double (&hrq)[4][2][4]) {
   double gqr[2][4], gt[2][4];            // gt[b][c] = G_I[r_c][q_b], from the tile of G_I at (rows r, columns q)
 #pragma unroll
@@ -94,13 +96,11 @@ __device__ __forceinline__ void tp_update(const uint8_t* sl, const uint32_t (&of
   }
   if (!DIAG) {
     // rows r_c = 2 lr + (c & 1) + 8 (c >> 1) of block 8 + wr; one 16-byte load gives (q_0, q_1) of a row.  offT is the
-    // offset of row 2 lr (+ 1 for `swap` lanes); the other row of the pair is at offT ^ 144 (next row, chunk bit 0
-    // flipped by the swizzle), rows + 8 are 1024 bytes further with the same swizzle phase.
+    // offset of row 2 lr; row 2 lr + 1 is at offT ^ 144 (next row, chunk bit 0 flipped by the swizzle), rows + 8 are
+    // 1024 bytes further with the same swizzle phase.
     const double2 t0 = lds128(sl, offT), t1 = lds128(sl, offT ^ 144), t2 = lds128(sl, offT + 1024), t3 = lds128(sl, (offT ^ 144) + 1024);
-    gt[0][0] = swap ? t1.x : t0.x; gt[1][0] = swap ? t1.y : t0.y;
-    gt[0][1] = swap ? t0.x : t1.x; gt[1][1] = swap ? t0.y : t1.y;
-    gt[0][2] = swap ? t3.x : t2.x; gt[1][2] = swap ? t3.y : t2.y;
-    gt[0][3] = swap ? t2.x : t3.x; gt[1][3] = swap ? t2.y : t3.y;
+    gt[0][0] = t0.x; gt[1][0] = t0.y; gt[0][1] = t1.x; gt[1][1] = t1.y;
+    gt[0][2] = t2.x; gt[1][2] = t2.y; gt[0][3] = t3.x; gt[1][3] = t3.y;
   }
 #pragma unroll
   for (int a = 0; a < 4; a++) {
@@ -133,7 +133,8 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int wp = warp >> 2, wq = (warp >> 1) & 1, wr = warp & 1;
-  const int lp = lane >> 4, lq = ((lane >> 2) & 1) * 2 + ((lane >> 3) & 1), lr = lane & 3;   // lane bit 2 -> q bit 2
+  // lane bits: 0-1 r offset, 2-3 q offset (pairs 0/3 and 1/2 inside a quarter-warp, see above), 4 p offset
+  const int lp = lane >> 4, lq = ((lane >> 3) & 1) ^ (((lane >> 2) & 1) * 3), lr = lane & 3;
   const int tp0 = wp * 8 + lp * 4;                      // 4 consecutive p
   const int tq0 = wq * 8 + lq * 2;                      // 2 consecutive q
   const int cq = tq0 >> 1;                              // 16-byte chunk of (.., tq0) in a 16-wide row
@@ -194,10 +195,10 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
     offQR[b] = (6 + wr) * TP_BLK_BYTES + row * 128 + ((lr ^ (row & 7)) << 4);
   }
 
-  const bool swap = (lane >> 2) & 1;                          // lanes whose q offset has bit 2 set (see tp_update)
-  const uint32_t offT = (((8 + wr) * TP_BLK_BYTES + (2 * lr) * 128 + ((cq ^ ((2 * lr) & 7)) << 4))) ^ (swap ? 144u : 0u);
+  const uint32_t offT = (8 + wr) * TP_BLK_BYTES + (2 * lr) * 128 + ((cq ^ ((2 * lr) & 7)) << 4);
 
   double hqr[4][2][4], hrq[4][2][4];
+  const int pf_stage = nS > 12 ? nS - 12 : 0;              // where the old H values are prefetched into L2
   int st = 0;                 // ring stage of the current iteration
   uint32_t par = 0;           // its mbarrier phase parity
   for (int k = 0; k < my_items; k++) {
@@ -210,16 +211,36 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
         for (int c = 0; c < 4; c++) hqr[a][b][c] = hrq[a][b][c] = 0.0;
 
     for (int s = 0; s < nS; s++) {
+      if (p.accumulate && s == pf_stage) {
+        // The read-modify-write of this item's H block at the end of the I loop is not overlapped with FMAs (one CTA per
+        // SM, every register in use): pull the old values into L2 a few stages ahead so that the reads of the write-back
+        // are L2 hits instead of a burst of DRAM reads (7 % of the launch at BASELINE config 4, where a chunk is 128 points).
+        const TripleItem nx = p.items[blockIdx.x + (long long)k * gridDim.x];
+        const long long sHp = (long long)p.NPp * p.NPp;
+        const int rA = nx.r0 + wr * 16 + 2 * lr;
+#pragma unroll
+        for (int a = 0; a < 4; a++) {
+          const double* Hp = p.H + (long long)(nx.p0 + tp0 + a) * sHp;
+          if (lr == 0) {                                     // one lane per 128-byte row segment of the direct block
+            prefetch_l2(Hp + (long long)(nx.q0 + tq0) * p.NPp + rA);
+            prefetch_l2(Hp + (long long)(nx.q0 + tq0 + 1) * p.NPp + rA);
+          }
+          if (!nx.diag && lq == 0) {                         // mirrored block: rows r, 16 q's = one line
+#pragma unroll
+            for (int c = 0; c < 4; c++) prefetch_l2(Hp + (long long)(rA + (c & 1) + 8 * (c >> 1)) * p.NPp + nx.q0 + tq0);
+          }
+        }
+      }
       mbar_wait(bar_full + 8 * st, par);
       if (tid == 0) fill();                          // TP_LOOKAHEAD stages ahead, two iterations behind the consumers
       __syncwarp();
       const uint8_t* sl = ring_ptr + st * TP_STAGE_BYTES;
       if (diag) {
 #pragma unroll 1
-        for (int ii = 0; ii < TP_IC; ii++) tp_update<true>(sl + ii * TP_SLICE_BYTES, offPQ, offPR, offQR, offT, swap, hqr, hrq);
+        for (int ii = 0; ii < TP_IC; ii++) tp_update<true>(sl + ii * TP_SLICE_BYTES, offPQ, offPR, offQR, offT, hqr, hrq);
       } else {
 #pragma unroll 1
-        for (int ii = 0; ii < TP_IC; ii++) tp_update<false>(sl + ii * TP_SLICE_BYTES, offPQ, offPR, offQR, offT, swap, hqr, hrq);
+        for (int ii = 0; ii < TP_IC; ii++) tp_update<false>(sl + ii * TP_SLICE_BYTES, offPQ, offPR, offQR, offT, hqr, hrq);
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(bar_empty + 8 * st);
