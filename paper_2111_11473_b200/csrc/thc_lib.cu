@@ -746,10 +746,11 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
       const double fo = (double)o, fv = (double)v, fNP = (double)NP, fNX = (double)NX;
       // measured on B200 (profiles/r02_final.md, config 4): one G pass (B_ia^I, its two half-transforms, A3 rebuilt when it
       // is not resident) runs at ~30 TFLOP/s = 9.6 s; the read-modify-write of H at the end of every work item of line 11
-      // is not overlapped with its FMAs and costs its HBM time at ~4 TB/s.
+      // is not overlapped with its FMAs and costs 6 % of a launch with 128-point chunks (17.9 vs 19.0 TFLOP/s), i.e. its
+      // bytes at ~7 TB/s.
       const double t_g = (fNX * (2 * fo * fv * fNX + 2 * fo * fv * fNP + 2 * fo * fNP * fNP) +
                           (NP * o * v * 8 > ((i64)4 << 30) ? 2 * fNP * fNP * fo * fv : 0.0)) / 30e12;            // DMMA, s
-      const double t_h = 16.0 * fNP * (double)pad_to(NP, 32) * (double)pad_to(NP, 32) / 4e12;            // HBM, s
+      const double t_h = 16.0 * fNP * (double)pad_to(NP, 32) * (double)pad_to(NP, 32) / 7e12;            // HBM, s
       double best = 1e300; int64_t bestX = 0, bestI = 0;
       // (chunks of a multiple of 128 grid points fill the 128-row tiles of the E_I / F_I products)
       for (int64_t bi : {16, 32, 64, 128, 256, 384, 512, 640, 768, 896, 1024}) {

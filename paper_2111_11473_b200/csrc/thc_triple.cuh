@@ -76,7 +76,6 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map
       "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
       ::"r"(dst), "l"(reinterpret_cast<uint64_t>(map)), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
 }
-__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 __device__ __forceinline__ double2 lds128(const uint8_t* base, uint32_t off) {
   return *reinterpret_cast<const double2*>(base + off);
 }
@@ -198,7 +197,6 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
   const uint32_t offT = (8 + wr) * TP_BLK_BYTES + (2 * lr) * 128 + ((cq ^ ((2 * lr) & 7)) << 4);
 
   double hqr[4][2][4], hrq[4][2][4];
-  const int pf_stage = nS > 12 ? nS - 12 : 0;              // where the old H values are prefetched into L2
   int st = 0;                 // ring stage of the current iteration
   uint32_t par = 0;           // its mbarrier phase parity
   for (int k = 0; k < my_items; k++) {
@@ -211,26 +209,6 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
         for (int c = 0; c < 4; c++) hqr[a][b][c] = hrq[a][b][c] = 0.0;
 
     for (int s = 0; s < nS; s++) {
-      if (p.accumulate && s == pf_stage) {
-        // The read-modify-write of this item's H block at the end of the I loop is not overlapped with FMAs (one CTA per
-        // SM, every register in use): pull the old values into L2 a few stages ahead so that the reads of the write-back
-        // are L2 hits instead of a burst of DRAM reads (7 % of the launch at BASELINE config 4, where a chunk is 128 points).
-        const TripleItem nx = p.items[blockIdx.x + (long long)k * gridDim.x];
-        const long long sHp = (long long)p.NPp * p.NPp;
-        const int rA = nx.r0 + wr * 16 + 2 * lr;
-#pragma unroll
-        for (int a = 0; a < 4; a++) {
-          const double* Hp = p.H + (long long)(nx.p0 + tp0 + a) * sHp;
-          if (lr == 0) {                                     // one lane per 128-byte row segment of the direct block
-            prefetch_l2(Hp + (long long)(nx.q0 + tq0) * p.NPp + rA);
-            prefetch_l2(Hp + (long long)(nx.q0 + tq0 + 1) * p.NPp + rA);
-          }
-          if (!nx.diag && lq == 0) {                         // mirrored block: rows r, 16 q's = one line
-#pragma unroll
-            for (int c = 0; c < 4; c++) prefetch_l2(Hp + (long long)(rA + (c & 1) + 8 * (c >> 1)) * p.NPp + nx.q0 + tq0);
-          }
-        }
-      }
       mbar_wait(bar_full + 8 * st, par);
       if (tid == 0) fill();                          // TP_LOOKAHEAD stages ahead, two iterations behind the consumers
       __syncwarp();
@@ -248,29 +226,48 @@ triple_product_kernel(const __grid_constant__ CUtensorMap mapE, const __grid_con
     }
 
     // ---- write back this item's block(s) of H[p][q][r] ---------------------------------------------------------------
+    // Accumulating launches (all I-chunks but the first) read the old values.  The old values of TWO p rows (32 doubles)
+    // are loaded before anything of those rows is stored: with one load -> add -> store chain per 16 bytes the compiler
+    // may not move a load above the preceding store, and 24 dependent round trips to L2 / HBM per work item cost 14 % of
+    // a launch at BASELINE config 4 (measured: 16.3 vs 19.0 TFLOP/s with / without accumulation).
     const TripleItem cur = p.items[blockIdx.x + (long long)k * gridDim.x];
     const long long sHp = (long long)p.NPp * p.NPp;
     const int rA = cur.r0 + wr * 16 + 2 * lr;              // r = rA, rA + 1, rA + 8, rA + 9
 #pragma unroll
-    for (int a = 0; a < 4; a++) {
-      double* Hp = p.H + (long long)(cur.p0 + tp0 + a) * sHp;
+    for (int a0 = 0; a0 < 4; a0 += 2) {
+      double2 od[2][2][2], om[2][4];
 #pragma unroll
-      for (int b = 0; b < 2; b++) {
-        double* row = Hp + (long long)(cur.q0 + tq0 + b) * p.NPp;
-        double2* d0 = reinterpret_cast<double2*>(row + rA);
-        double2* d1 = reinterpret_cast<double2*>(row + rA + 8);
-        double2 v0 = make_double2(hqr[a][b][0], hqr[a][b][1]), v1 = make_double2(hqr[a][b][2], hqr[a][b][3]);
-        if (p.accumulate) { double2 o0 = *d0, o1 = *d1; v0.x += o0.x; v0.y += o0.y; v1.x += o1.x; v1.y += o1.y; }
-        *d0 = v0; *d1 = v1;
-      }
-      if (!cur.diag) {
+      for (int aa = 0; aa < 2; aa++) {
+        double* Hp = p.H + (long long)(cur.p0 + tp0 + a0 + aa) * sHp;
+#pragma unroll
+        for (int b = 0; b < 2; b++) {
+          const double* row = Hp + (long long)(cur.q0 + tq0 + b) * p.NPp + rA;
+          od[aa][b][0] = od[aa][b][1] = make_double2(0.0, 0.0);
+          if (p.accumulate) { od[aa][b][0] = *reinterpret_cast<const double2*>(row); od[aa][b][1] = *reinterpret_cast<const double2*>(row + 8); }
+        }
 #pragma unroll
         for (int c = 0; c < 4; c++) {
-          const int r = rA + (c & 1) + 8 * (c >> 1);
-          double2* d = reinterpret_cast<double2*>(Hp + (long long)r * p.NPp + cur.q0 + tq0);
-          double2 vv = make_double2(hrq[a][0][c], hrq[a][1][c]);
-          if (p.accumulate) { double2 o = *d; vv.x += o.x; vv.y += o.y; }
-          *d = vv;
+          om[aa][c] = make_double2(0.0, 0.0);
+          if (p.accumulate && !cur.diag)
+            om[aa][c] = *reinterpret_cast<const double2*>(Hp + (long long)(rA + (c & 1) + 8 * (c >> 1)) * p.NPp + cur.q0 + tq0);
+        }
+      }
+#pragma unroll
+      for (int aa = 0; aa < 2; aa++) {
+        const int a = a0 + aa;
+        double* Hp = p.H + (long long)(cur.p0 + tp0 + a) * sHp;
+#pragma unroll
+        for (int b = 0; b < 2; b++) {
+          double* row = Hp + (long long)(cur.q0 + tq0 + b) * p.NPp + rA;
+          *reinterpret_cast<double2*>(row) = make_double2(hqr[a][b][0] + od[aa][b][0].x, hqr[a][b][1] + od[aa][b][0].y);
+          *reinterpret_cast<double2*>(row + 8) = make_double2(hqr[a][b][2] + od[aa][b][1].x, hqr[a][b][3] + od[aa][b][1].y);
+        }
+        if (!cur.diag) {
+#pragma unroll
+          for (int c = 0; c < 4; c++) {
+            double2* d = reinterpret_cast<double2*>(Hp + (long long)(rA + (c & 1) + 8 * (c >> 1)) * p.NPp + cur.q0 + tq0);
+            *d = make_double2(hrq[a][0][c] + om[aa][c].x, hrq[a][1][c] + om[aa][c].y);
+          }
         }
       }
     }
