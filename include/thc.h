@@ -94,7 +94,10 @@ typedef struct {
   int32_t use_graph;        /* 1 = capture the evaluation into a CUDA graph on first use and replay it while the */
                             /* pointers stay the same (launch-bound small shapes); 0 = never; -1 = auto: on when */
                             /* the shape is launch-bound (< 2e10 algorithmic flop) and B_vv is resident          */
-  int32_t reserved;         /* must be 0                                                                    */
+  int32_t t2sq_algorithm;   /* how the ladder-type T2^2 terms (sigma6, Eqs.32+33) are evaluated: 4 = the O(N^4) Alg.6  */
+                            /* (THC ERIs + the line-11 kernel), 5 = the O(N^5) GEMM-only Alg.4 + Alg.5, 0 = auto: the */
+                            /* cheaper one by a flop/rate model ("ideally one would ..."); sharded      */
+                            /* evaluations always use Alg.6                                                          */
 } thc_options;
 
 /* Create a handle for one problem shape.  (o, v, NL, NP, NX) as in BASELINE.json / PAPER.md l.47-54

@@ -56,7 +56,7 @@ class _Options(ctypes.Structure):
     _fields_ = [("bL", ctypes.c_int64), ("bP7", ctypes.c_int64), ("bX", ctypes.c_int64), ("bI", ctypes.c_int64),
                 ("workspace_bytes_max", ctypes.c_int64), ("tma_min_flop", ctypes.c_int64), ("term_mask", ctypes.c_int32), ("device", ctypes.c_int32),
                 ("bvv_mode", ctypes.c_int32), ("check_symmetry", ctypes.c_int32), ("use_graph", ctypes.c_int32),
-                ("reserved", ctypes.c_int32)]
+                ("t2sq_algorithm", ctypes.c_int32)]
 
 
 BVV_MODES = dict(device=0, host=1, provider=2)
@@ -169,7 +169,8 @@ class Thc:
     """One problem shape (thc_setup ... thc_destroy).  Methods mirror the C entry points."""
 
     def __init__(self, o, v, NL, NP, NX, *, bL=0, bP7=0, bX=0, bI=0, workspace_bytes_max=0, term_mask=0,
-                 device=-1, torch_workspace=True, bvv_mode="device", check_symmetry=False, use_graph=-1, tma_min_flop=0):
+                 device=-1, torch_workspace=True, bvv_mode="device", check_symmetry=False, use_graph=-1, tma_min_flop=0,
+                 t2sq_algorithm=0):
         import torch
         if not torch.cuda.is_available():
             raise ThcError("no CUDA device: the THC residual has no CPU path")
@@ -177,7 +178,7 @@ class Thc:
         self._h = ctypes.c_void_p()
         self.bvv_mode = bvv_mode
         opt = _Options(bL, bP7, bX, bI, workspace_bytes_max, tma_min_flop, term_mask, device, BVV_MODES[bvv_mode],
-                       int(bool(check_symmetry)), int(use_graph), 0)
+                       int(bool(check_symmetry)), int(use_graph), int(t2sq_algorithm))
         _check(lib().thc_setup(ctypes.byref(self._h), o, v, NL, NP, NX, ctypes.byref(opt)))
         self._ws = None
         self._torch_ws = torch_workspace

@@ -33,6 +33,7 @@ struct thc_handle {
   uint64_t gemm_smem_mask, ring_smem_mask;   // same, one bit per dgemm_kernel / ring_fused_kernel instantiation
   double tma_min_flop;               // GEMMs of at least this many flop may use the TMA-fed kernel (< 0: never)
   int32_t check_symmetry;
+  int32_t t2sq_algorithm;            // 4 or 5 (resolved in thc_setup)
   // Alg.6 line 11: work-item lists (device memory owned by the handle), one per (nPp, NPp) shape seen
   struct TripleList { int64_t nPp, NPp; thc::TripleItem* dev; int n; };
   std::vector<TripleList> tp_lists;
@@ -449,6 +450,9 @@ struct Ctx {
     prof_stop(2);
   }
   void t1_eps(const double* eps, const double* t1, double* out, i64 o, i64 v) { THC_EW(t1_eps_kernel, o * v, 24.0 * o * v, eps, t1, out, (int)o, (int)v); }
+  void pair_accumulate(const double* J, const double* FA, i64 ldfa, const double* FB, i64 ldfb, double* out, i64 n, i64 n1, i64 n2) {
+    THC_EW(pair_accumulate_kernel, n * n, 8.0 * n * n * (n1 * n2 + 2.0), J, FA, ldfa, FB, ldfb, out, (int)n, (int)n1, (int)n2);
+  }
   void diag(const double* A, double* d, i64 n) { THC_EW(diag_kernel, n, 16.0 * n, A, d, (int)n); }
   void copy(const double* src, double* dst, i64 n) {
     if (dry || !ok()) return;

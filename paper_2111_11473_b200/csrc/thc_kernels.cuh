@@ -70,6 +70,24 @@ __global__ void t1_eps_kernel(const double* __restrict__ eps, const double* __re
   }
 }
 
+// Alg.4 / Alg.5 line 13 (l.640, l.677): sigma^{XX'} += sum_pairs J_pair^{XX'} fa_pair[X] fb_pair[X'] for the n1 x n2 pairs
+// (i1, i2) of a block; J is [(i1, i2)][n][n], fa = FA[i1][.], fb = FB[i2][.] (A^{XX'} = y^X y^{X'} of line 3).
+__global__ void pair_accumulate_kernel(const double* __restrict__ J, const double* __restrict__ FA, i64 ldfa,
+                                       const double* __restrict__ FB, i64 ldfb, double* __restrict__ out, int n, int n1, int n2) {
+  const i64 nn = (i64)n * n;
+  THC_GRID_STRIDE(idx, nn) {
+    const int X = (int)(idx / n), Xp = (int)(idx % n);
+    double s = 0.0;
+    for (int i1 = 0; i1 < n1; i1++) {
+      const double fa = FA[(i64)i1 * ldfa + X];
+      double s1 = 0.0;
+      for (int i2 = 0; i2 < n2; i2++) s1 = fma(J[((i64)i1 * n2 + i2) * nn + idx], FB[(i64)i2 * ldfb + Xp], s1);
+      s = fma(fa, s1, s);
+    }
+    out[idx] += s;
+  }
+}
+
 // d[P] = A[P][P]
 __global__ void diag_kernel(const double* __restrict__ A, double* __restrict__ d, int n) {
   THC_GRID_STRIDE(idx, (i64)n) d[idx] = A[idx * n + idx];

@@ -674,7 +674,8 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
   if (!hp) return THC_ERR_INVALID_ARG;
   *hp = nullptr;
   if (o <= 0 || v <= 0 || NL <= 0 || NP <= 0 || NX <= 0) return THC_ERR_INVALID_ARG;
-  if (opt && (opt->bvv_mode < 0 || opt->bvv_mode > 2 || opt->reserved != 0 || opt->use_graph < -1 || opt->use_graph > 1))
+  if (opt && (opt->bvv_mode < 0 || opt->bvv_mode > 2 || opt->use_graph < -1 || opt->use_graph > 1 ||
+              (opt->t2sq_algorithm != 0 && opt->t2sq_algorithm != 4 && opt->t2sq_algorithm != 5)))
     return THC_ERR_INVALID_ARG;
   if (opt && (opt->bL < 0 || opt->bP7 < 0 || opt->bX < 0 || opt->bI < 0 || opt->workspace_bytes_max < 0)) return THC_ERR_INVALID_ARG;
   const int64_t lim = (int64_t)1 << 31;
@@ -702,6 +703,7 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
   h->launches = 0; h->last_cuda = 0; h->smem_configured = false;
   h->gemm_smem_mask = 0; h->ring_smem_mask = 0; h->tma_min_flop = (opt && opt->tma_min_flop) ? (double)opt->tma_min_flop : 2e8;
   h->check_symmetry = opt ? opt->check_symmetry : 0; h->sym_scratch = nullptr;
+  h->t2sq_algorithm = 4;                       // resolved below once the sizes are known
   h->prof_mask = 0; h->prof_used = 0; h->prof_done = 0; h->encode_tiled = nullptr;
   h->cap_stream = nullptr;
   {
