@@ -55,6 +55,83 @@ struct PackedLayout {
 
 inline i64 pad_to(i64 x, i64 m) { return (x + m - 1) / m * m; }
 
+// O(N^5) GEMM-only evaluation of the ladder-type T2^2 terms: PAPER.md Alg.4 (Eq.32, l.608-643) and Alg.5 (Eq.33,
+// l.645-680), the variant the paper prefers for small molecules (l.250, l.309).  Every line of the listings is a GEMM
+// batched over a block of pairs -- (i, j) for Alg.4, (a, j) for Alg.5 -- with the Hadamard products of lines 4, 7, 10 fused
+// into GEMM epilogues (aux) and line 13 done by pair_accumulate_kernel.  Lines 3-5 of both algorithms are the explicit
+// amplitudes of the pair, t_ij^cd and t_lj^ad, formed from the scaled factors XS[(i,a)][P] = Xo[i,P] Xv[a,P].
+void plan_s6_n5(Ctx& c, const Inputs& in, double* s6, const double* XoT, const double* XvT, const double* YoT, const double* YvT) {
+  thc_handle* h = c.h;
+  thc::Arena& ar = c.ar;
+  const i64 o = h->o, v = h->v, NP = h->NP, NX = h->NX, NP2 = NP * NP, ov = o * v;
+  const double* Yo = in.Y;
+  const double* Yv = in.Y + o * NX;
+  const double *Z = in.Z, *V = in.V, *Xo = in.Xo, *Xv = in.Xv;
+  const i64 m0 = ar.mark();
+  c.fill(s6, NP2, 0.0);
+  double* XS = ar.alloc(ov * NP);
+  c.rowscale(Xv, NP, Xo, NP, nullptr, 1.0, XS, o, v, NP);                       // XS[(i,a)][P]
+  double *E = ar.alloc(o * NX * NX), *W = ar.alloc(o * o * NX);                // one i (or a) at a time: lines 6-8
+  const i64 budget = (i64)3 << 30;                                              // bytes of per-block intermediates
+  // ---- Alg.4: pairs (i, j), blocks of ni values of i -------------------------------------------------------------------------
+  {
+    const i64 per = 8 * (v * NP + v * ov + v * o * NX + o * o * o + o * o * NP + o * NP2 + ov * NP + ov * v);
+    const i64 bi = std::max<i64>(1, std::min<i64>(o, budget / per));
+    for (i64 i0 = 0; i0 < o; i0 += bi) {
+      const i64 ni = std::min<i64>(bi, o - i0), m1 = ar.mark();
+      double *A3b = ar.alloc(ni * v * NP), *T4 = ar.alloc(ni * v * ov), *U1 = ar.alloc(ni * v * o * NX), *X4 = ar.alloc(ni * o * o * o);
+      c.gemm(Gemm(XS + i0 * v * NP, NP, 'K', Z, NP, 'K', A3b, NP, ni * v, NP, NP));             // lines 3-4: T .* A folded into XS Z
+      c.gemm(Gemm(A3b, NP, 'K', XS, NP, 'K', T4, ov, ni * v, ov, NP));                         // line 5: T4[(i,c)][(j,d)] = t_ij^cd
+      c.gemm(Gemm(T4, v, 'K', YvT, v, 'K', U1, NX, ni * v * o, NX, v));                        // line 6, first half: sum_d
+      for (i64 ii = 0; ii < ni; ii++) {
+        // line 6 (second half) + line 7: E^{IJ} = z^{IJ} sum_c x_c^I U1[(i,c,j)][J], batch over j
+        c.gemm(Gemm(YvT, v, 'K', U1 + ii * v * o * NX, o * NX, 'N', E, NX, NX, NX, v).batch(o, 0, NX, NX * NX).aux(V, NX, 0));
+        // line 8: F_kl = sum_IJ E^{IJ} x_k^I x_l^J
+        c.gemm(Gemm(Yo, NX, 'K', E, NX, 'N', W, NX, o, NX, NX).batch(o, 0, NX * NX, o * NX));
+        c.gemm(Gemm(W, NX, 'K', Yo, NX, 'K', X4 + ii * o * o * o, o, o * o, o, NX));
+      }
+      double *FX = ar.alloc(ni * o * o * NP), *Hb = ar.alloc(ni * o * NP2), *HX = ar.alloc(ni * ov * NP), *I4 = ar.alloc(ni * ov * v);
+      c.gemm(Gemm(X4, o, 'K', XoT, o, 'K', FX, NP, ni * o * o, NP, o));                        // line 9, first half: sum_l
+      c.gemm(Gemm(Xo, NP, 'M', FX, NP, 'N', Hb, NP, NP, NP, o).batch(ni * o, 0, o * NP, NP2).aux(Z, NP, 0));   // lines 9-10: H = T .* G
+      c.gemm(Gemm(Xv, NP, 'K', Hb, NP, 'N', HX, NP, v, NP, NP).batch(ni * o, 0, NP2, v * NP));                  // line 11: sum_Y
+      c.gemm(Gemm(HX, NP, 'K', Xv, NP, 'K', I4, v, ni * ov, v, NP));                                          //          sum_Y' -> I_ab
+      c.gemm(Gemm(I4, v, 'K', XvT, v, 'K', HX, NP, ni * ov, NP, v));                                          // line 12: sum_b
+      c.gemm(Gemm(Xv, NP, 'M', HX, NP, 'N', Hb, NP, NP, NP, v).batch(ni * o, 0, v * NP, NP2));                  //          sum_a -> J^{XX'}
+      c.pair_accumulate(Hb, Xo + i0 * NP, NP, Xo, NP, s6, NP, ni, o);                                          // line 13
+      ar.release(m1);
+    }
+  }
+  // ---- Alg.5: pairs (a, j), blocks of na values of a -------------------------------------------------------------------------
+  {
+    const i64 per = 8 * (2 * o * NP + o * ov + o * o * NX + o * ov + 2 * o * o * NP + o * NP2 + o * ov);
+    const i64 ba = std::max<i64>(1, std::min<i64>(v, budget / per));
+    for (i64 a0 = 0; a0 < v; a0 += ba) {
+      const i64 na = std::min<i64>(ba, v - a0), m1 = ar.mark();
+      double *XSa = ar.alloc(na * o * NP), *A3a = ar.alloc(na * o * NP), *T4a = ar.alloc(na * o * ov), *U5 = ar.alloc(na * o * o * NX);
+      double* F5 = ar.alloc(na * o * ov);
+      c.rowscale(Xo, NP, Xv + a0 * NP, NP, nullptr, 1.0, XSa, na, o, NP);                       // XSa[(a,l)][P]
+      c.gemm(Gemm(XSa, NP, 'K', Z, NP, 'K', A3a, NP, na * o, NP, NP));
+      c.gemm(Gemm(A3a, NP, 'K', XS, NP, 'K', T4a, ov, na * o, ov, NP));                        // lines 3-5: T4a[(a,l)][(j,d)] = t_lj^ad
+      c.gemm(Gemm(T4a, v, 'K', YvT, v, 'K', U5, NX, na * o * o, NX, v));                       // line 6, first half: sum_d
+      for (i64 aa = 0; aa < na; aa++) {
+        c.gemm(Gemm(YoT, o, 'K', U5 + aa * o * o * NX, o * NX, 'N', E, NX, NX, NX, o).batch(o, 0, NX, NX * NX).aux(V, NX, 0));   // lines 6-7
+        c.gemm(Gemm(Yo, NX, 'K', E, NX, 'K', W, NX, o, NX, NX).batch(o, 0, NX * NX, o * NX));                               // line 8: sum_J x_k^J
+        c.gemm(Gemm(W, NX, 'K', Yv, NX, 'K', F5 + aa * o * ov, v, o * o, v, NX));                                          //         sum_I x_c^I
+      }
+      double *FY = ar.alloc(na * o * o * NP), *Hb = ar.alloc(na * o * NP2), *HX = ar.alloc(na * o * o * NP), *I5 = ar.alloc(na * o * ov);
+      c.gemm(Gemm(F5, v, 'K', XvT, v, 'K', FY, NP, na * o * o, NP, v));                        // line 9, first half: sum_c
+      c.gemm(Gemm(FY, NP, 'M', Xo, NP, 'N', Hb, NP, NP, NP, o).batch(na * o, o * NP, 0, NP2).aux(Z, NP, 0));   // lines 9-10
+      c.gemm(Gemm(Xo, NP, 'K', Hb, NP, 'N', HX, NP, o, NP, NP).batch(na * o, 0, NP2, o * NP));                  // line 11: sum_Y y_i^Y
+      c.gemm(Gemm(HX, NP, 'K', Xv, NP, 'K', I5, v, na * o * o, v, NP));                                        //          sum_Y' y_b^Y' -> I_ib
+      c.gemm(Gemm(I5, v, 'K', XvT, v, 'K', HX, NP, na * o * o, NP, v));                                        // line 12: sum_b
+      c.gemm(Gemm(Xo, NP, 'M', HX, NP, 'N', Hb, NP, NP, NP, o).batch(na * o, 0, o * NP, NP2));                  //          sum_i -> J^{XX'}
+      c.pair_accumulate(Hb, Xv + a0 * NP, NP, Xo, NP, s6, NP, na, o);                                          // line 13: A = y_a^X y_j^X'
+      ar.release(m1);
+    }
+  }
+  ar.release(m0);
+}
+
 // The whole residual evaluation.  Runs either for real or dry (workspace sizing); both take identical branches.
 void plan_residual(Ctx& c, const Inputs& in, const Outputs& out, const Shard& sh = Shard()) {
   thc_handle* h = c.h;
@@ -365,7 +442,9 @@ void plan_residual(Ctx& c, const Inputs& in, const Outputs& out, const Shard& sh
   }
 
   // ---- H9: Alg.6, ladder-type T2^2 terms with THC ERIs (Eq.34 l.254) -------------------------------------------------
-  if (do_s6 && local) {
+  if (do_s6 && sh.phase == 0 && h->t2sq_algorithm == 5) {
+    plan_s6_n5(c, in, s6, XoT, XvT, YoT, YvT);
+  } else if (do_s6 && local) {
     const i64 m0 = ar.mark();
     const i64 NPp = pad_to(NP, thc::TP_RT);
     // line 1: A3[Q][i][a] = sum_S Z[Q,S] Xo[i,S] Xv[a,S].  It only feeds lines 4-5 at the start of a row block.  While it
@@ -703,7 +782,19 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
   h->launches = 0; h->last_cuda = 0; h->smem_configured = false;
   h->gemm_smem_mask = 0; h->ring_smem_mask = 0; h->tma_min_flop = (opt && opt->tma_min_flop) ? (double)opt->tma_min_flop : 2e8;
   h->check_symmetry = opt ? opt->check_symmetry : 0; h->sym_scratch = nullptr;
-  h->t2sq_algorithm = 4;                       // resolved below once the sizes are known
+  {
+    // Alg.6 vs Alg.4+5 ("ideally one would..."): leading flop counts over measured rates (line 11 ~17
+    // TFLOP/s, GEMMs of a G pass ~30, the many small batched products of Alg.4/5 ~12: 7.5 at config 1, 14 at config 2)
+    // plus ~5 us per launch (Alg.4/5 loop over i and a).  Measured sigma6 times, Alg.6 / Alg.4+5: config 0 0.26 / 0.92 ms,
+    // config 1 7.3 / 20.3 ms, config 2 0.64 / 2.36 s -- on B200 the crossover the paper saw on V100 is below config 0.
+    const double fo = (double)o, fv = (double)v, fP = (double)NP, fX = (double)NX;
+    const double t4 = 5 * fX * fP * fP * fP / 17e12 + (2 * (fo + fv) * fP * fP * fX + fX * (2 * fo * fv * fP + 2 * fo * fP * fP + 2 * fo * fv * fX)) / 30e12 + 5e-6 * 20;
+    const double t5 = (fo * fo * (2 * fv * fX * fX + 2 * fo * fX * fX + 2 * fo * fP * fP + 4 * fv * fP * fP + 2 * fv * fv * (fX + 2 * fP)) +
+                       fo * fv * (4 * fo * fX * fX + 6 * fo * fP * fP + 2 * fo * fv * (fX + 2 * fP))) / 12e12 + 5e-6 * (3 * (fo + fv) + 30);
+    const int want = opt ? opt->t2sq_algorithm : 0;
+    const bool n5_fits = (double)o * NX * NX * 8 < 8e9;
+    h->t2sq_algorithm = want ? want : ((t5 < t4 && n5_fits) ? 5 : 4);
+  }
   h->prof_mask = 0; h->prof_used = 0; h->prof_done = 0; h->encode_tiled = nullptr;
   h->cap_stream = nullptr;
   {

@@ -219,3 +219,19 @@ def test_probe_reports_plausible_ceilings():
     h.close()
     assert 20.0 < p["dmma_tflops"] < 60.0 and 20.0 < p["dfma_tflops"] < 60.0, p
     assert 60.0 < p["lds128_bytes_per_clk_per_sm"] <= 140.0, p
+
+
+@pytest.mark.parametrize("dims", [(3, 4, 6, 5, 7), (7, 13, 19, 37, 45), (6, 18, 10, 64, 96), (20, 9, 5, 33, 40)])
+def test_n5_gemm_only_t2sq_variant(dims):
+    """sigma6 through the O(N^5) GEMM-only Alg.4 + Alg.5 instead of Alg.6: same oracle, same
+    tolerance, O(1) amplitudes so that the term is not negligible; both variants forced explicitly."""
+    x = small_inputs(*dims, seed=19, zmul=30.0)
+    ref = oracle_eval(x)
+    _check_against(x, ref, t2sq_algorithm=5)
+    _check_against(x, ref, t2sq_algorithm=4)
+
+
+def test_n5_variant_config0_and_config1(oracle_cfg):
+    for cfg in (0, 1):
+        x, ref = oracle_cfg(cfg)
+        _check_against(x, ref, t2sq_algorithm=5)
