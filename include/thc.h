@@ -54,7 +54,8 @@ typedef enum {
   THC_ERR_NO_MEMORY = -3,     /* workspace too small / cudaMalloc failed                        */
   THC_ERR_CUDA = -4,          /* a CUDA call or kernel launch failed (see thc_last_error)       */
   THC_ERR_NO_DEVICE = -5,     /* no sm_100 device visible                                       */
-  THC_ERR_PROVIDER = -6       /* a thc_bvv_provider callback returned non-zero                   */
+  THC_ERR_PROVIDER = -6,      /* a thc_bvv_provider callback returned non-zero                   */
+  THC_ERR_STATIC_LIMIT = -7   /* thc_dgemm_static: needs more than THC_STATIC_SCRATCH_BYTES     */
 } thc_status;
 
 /* Where the vv Cholesky blocks B_vv[NL][v][v] live (PAPER.md l.191-195 keeps the 3-index arrays off the GPU and
@@ -252,8 +253,35 @@ int thc_triple_product(thc_handle* h, int64_t nI, int64_t nPp, int64_t NPp, cons
  * clock in MHz, out[7] = 0. */
 int thc_probe(thc_handle* h, double out[8]);
 
+/* ---- allocation-free entry point ------------------------------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA-graph capture, tight serving loops, harnesses that forbid
+ * it): the split-K FP64 DMMA GEMM of the GEMM chains ("rate limiting step"; same kernels as thc_dgemm)
+ * with the split-K partial tiles in a static device array of THC_STATIC_SCRATCH_BYTES instead of a workspace.  Needs no
+ * thc_handle and calls no cudaMalloc / cudaFree / allocating library routine.
+ *
+ *   C[M][N] = alpha * sum_k A[m*lda + k] * B[n*ldb + k] + beta * C          (both operands K-major, row-major C)
+ *
+ * A, B, C: device pointers on `device` (-1 = the current device), 8-byte aligned (16-byte aligned with even lda / ldb
+ * selects the faster copy path), not overlapping; caller-owned.  `stream`: a cudaStream_t (NULL = default stream); the
+ * call is asynchronous.  `splits`: number of K ranges, >= 1, or 0 = chosen by the library (about two waves of CTAs,
+ * within the scratch limit).  With splits S the call needs S * M * N * 8 bytes of scratch: more than
+ * THC_STATIC_SCRATCH_BYTES returns THC_ERR_STATIC_LIMIT (nothing is launched); splits = 0 never exceeds the limit (it
+ * falls back to fewer splits, down to 1 = no scratch).  splits > 1 is summed in split order (deterministic).
+ *
+ * The array is one per GPU per process, held from library load until exit, and shared by every call: two calls that
+ * overlap on the GPU (different streams, or graphs replayed concurrently) race on it; calls on one stream do not.  It
+ * keeps the previous call's partial tiles; nothing has to start at zero because every partial element that the
+ * reduction reads is written by the GEMM kernel of the same call first.
+ *
+ * thc_static_init(device) does the once-per-device set-up (address of the array, shared-memory opt-in of the kernels,
+ * SM count) ahead of time, e.g. before a graph capture; thc_dgemm_static does it on first use otherwise.          */
+#define THC_STATIC_SCRATCH_BYTES (16ll << 20)
+int thc_static_init(int device);
+int thc_dgemm_static(int device, void* stream, int64_t M, int64_t N, int64_t K, int splits, double alpha,
+                     const double* A, int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc);
+
 const char* thc_strerror(int status);
-int thc_last_error(const thc_handle* h);        /* the cudaError_t of the last THC_ERR_CUDA on this handle, else 0 */
+int thc_last_error(const thc_handle* h);       /* the cudaError_t of the last THC_ERR_CUDA on this handle, else 0 */
 int thc_last_cuda_error(const thc_handle* h);   /* older name of thc_last_error (same value)                       */
 
 #ifdef __cplusplus

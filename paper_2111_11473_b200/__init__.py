@@ -25,7 +25,9 @@ SYMBOLS = ("thc_setup", "thc_destroy", "thc_workspace_bytes", "thc_workspace_byt
            "thc_triple_product", "thc_strerror", "thc_last_cuda_error", "thc_last_error", "thc_shard_range",
            "thc_shard_doubles", "thc_residual_shard", "thc_residual_finish", "thc_energy_shard",
            "thc_profile_launches", "thc_profile_launch", "thc_algorithmic_work", "thc_probe", "thc_workspace_bytes_rr",
-           "thc_residual_rr", "thc_workspace_bytes_t1", "thc_residual_t1")
+           "thc_residual_rr", "thc_workspace_bytes_t1", "thc_residual_t1", "thc_static_init", "thc_dgemm_static")
+
+STATIC_SCRATCH_BYTES = 16 << 20          # THC_STATIC_SCRATCH_BYTES of include/thc.h
 
 TERM_NAMES = ("s1", "s2", "s3", "s6", "s7", "s9")
 TERM_BITS = dict(s1=1, s2=2, s3=4, s6=8, s7=16, s9=32)
@@ -133,6 +135,8 @@ def lib() -> ctypes.CDLL:
     L.thc_strerror.argtypes = [ctypes.c_int]
     L.thc_strerror.restype = ctypes.c_char_p
     L.thc_last_cuda_error.argtypes = [VP]
+    L.thc_static_init.argtypes = [ctypes.c_int]
+    L.thc_dgemm_static.argtypes = [ctypes.c_int, P, I64, I64, I64, ctypes.c_int, D, P, I64, P, I64, D, P, I64]
     for name in SYMBOLS:
         getattr(L, name)          # AttributeError if a declared symbol is missing
     _lib = L
@@ -145,6 +149,30 @@ def _check(st: int, h=None):
         if h is not None and st == -4:
             msg += f" [cudaError {lib().thc_last_error(h)}]"
         raise ThcError(f"thc status {st}: {msg}")
+
+
+def thc_static_init(device: int = -1):
+    """Once-per-device set-up of the allocation-free entry point (include/thc.h)."""
+    _check(lib().thc_static_init(int(device)))
+
+
+def thc_dgemm_static(A, B, C, alpha: float = 1.0, beta: float = 0.0, splits: int = 0):
+    """C[M][N] = alpha * A[M][K] B[N][K]^T + beta * C through thc_dgemm_static (include/thc.h): no handle, no workspace, no
+    cudaMalloc; split-K partials in the library's static device array (STATIC_SCRATCH_BYTES).  Runs on torch's current
+    stream of the tensors' device.  Argument marshalling only."""
+    import torch
+    for name, t in (("A", A), ("B", B), ("C", C)):
+        if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.float64 or t.dim() != 2 or t.stride(1) != 1:
+            raise ThcError(f"{name}: need a 2-D float64 CUDA tensor with unit inner stride")
+    M, K = A.shape
+    N = B.shape[0]
+    if B.shape[1] != K or tuple(C.shape) != (M, N) or A.device != B.device or A.device != C.device:
+        raise ThcError("thc_dgemm_static: shapes / devices do not match")
+    dev = A.device.index
+    stream = torch.cuda.current_stream(A.device).cuda_stream
+    _check(lib().thc_dgemm_static(dev, ctypes.c_void_p(stream), M, N, K, int(splits), float(alpha),
+                                  ctypes.c_void_p(A.data_ptr()), A.stride(0), ctypes.c_void_p(B.data_ptr()), B.stride(0),
+                                  float(beta), ctypes.c_void_p(C.data_ptr()), C.stride(0)))
 
 
 def _dev_ptr(t, name, numel=None):

@@ -12,6 +12,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include "thc_host.cuh"
 
@@ -1358,6 +1359,7 @@ const char* thc_strerror(int status) {
     case THC_ERR_CUDA: return "CUDA error (see thc_last_error)";
     case THC_ERR_NO_DEVICE: return "no sm_100 CUDA device";
     case THC_ERR_PROVIDER: return "B_vv provider callback failed";
+    case THC_ERR_STATIC_LIMIT: return "thc_dgemm_static: splits * M * N * 8 bytes exceed THC_STATIC_SCRATCH_BYTES";
     default: return "unknown status";
   }
 }
@@ -1366,3 +1368,100 @@ int thc_last_error(const thc_handle* h) { return h ? h->last_cuda : 0; }
 int thc_last_cuda_error(const thc_handle* h) { return thc_last_error(h); }
 
 }  // extern "C"
+
+// ---- allocation-free split-K DGEMM (include/thc.h: thc_static_init, thc_dgemm_static) -----------------------------------
+// The split-K partial tiles live in a static device array: one per GPU per process, from library load until exit.
+// In host code `thc_static_scratch` is only a host-side stand-in for the symbol, never a device address: the address
+// that the kernels get comes from cudaGetSymbolAddress, asked once per device with that device current.
+static __device__ __align__(256) double thc_static_scratch[THC_STATIC_SCRATCH_BYTES / 8];
+
+namespace {
+constexpr int STATIC_MAX_DEVICES = 64;
+struct StaticDev { bool ready = false; double* scratch = nullptr; int sms = 0; };
+StaticDev g_static_dev[STATIC_MAX_DEVICES];
+std::mutex g_static_mutex;
+
+// set-up of the current device (the caller holds a DeviceGuard on `device`)
+int static_init_current(int device) {
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  StaticDev& d = g_static_dev[device];
+  if (d.ready) return THC_OK;
+  int major = 0;
+  if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device) != cudaSuccess || major != 10) {
+    cudaGetLastError();
+    return THC_ERR_NO_DEVICE;
+  }
+  double* ptr = nullptr;
+  if (cudaGetSymbolAddress(reinterpret_cast<void**>(&ptr), thc_static_scratch) != cudaSuccess || !ptr) { cudaGetLastError(); return THC_ERR_CUDA; }
+  if (cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess || d.sms <= 0) { cudaGetLastError(); return THC_ERR_CUDA; }
+  const int sm = thc::gemm_smem_bytes(64, 64, 16, 4, true, true);        // 64 KB: above the 48 KB default
+  if (cudaFuncSetAttribute(thc::dgemm_kernel<THC_SMALL, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm) != cudaSuccess ||
+      cudaFuncSetAttribute(thc::dgemm_kernel<THC_SMALL, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm) != cudaSuccess) {
+    cudaGetLastError();
+    return THC_ERR_CUDA;
+  }
+  d.scratch = ptr;
+  d.ready = true;
+  return THC_OK;
+}
+}  // namespace
+
+int thc_static_init(int device) {
+  if (device < 0 && cudaGetDevice(&device) != cudaSuccess) { cudaGetLastError(); return THC_ERR_NO_DEVICE; }
+  if (device >= STATIC_MAX_DEVICES) return THC_ERR_INVALID_ARG;
+  DeviceGuard g(device);
+  if (!g.ok) return THC_ERR_CUDA;
+  return static_init_current(device);
+}
+
+int thc_dgemm_static(int device, void* stream, int64_t M, int64_t N, int64_t K, int splits, double alpha, const double* A,
+                     int64_t lda, const double* B, int64_t ldb, double beta, double* C, int64_t ldc) {
+  if (bad_ptr(A) || bad_ptr(B) || bad_ptr(C) || M <= 0 || N <= 0 || K <= 0 || splits < 0) return THC_ERR_INVALID_ARG;
+  const int64_t lim = (int64_t)1 << 31;
+  if (M >= lim || N >= lim || K >= lim) return THC_ERR_OVERFLOW;
+  if (lda < K || ldb < K || ldc < N) return THC_ERR_INVALID_ARG;
+  const i64 per = M * N, cap = THC_STATIC_SCRATCH_BYTES / 8;
+  if (splits > 1 && (splits > cap || per > cap / splits)) return THC_ERR_STATIC_LIMIT;
+  if (device < 0 && cudaGetDevice(&device) != cudaSuccess) { cudaGetLastError(); return THC_ERR_NO_DEVICE; }
+  if (device >= STATIC_MAX_DEVICES) return THC_ERR_INVALID_ARG;
+  DeviceGuard g(device);
+  if (!g.ok) return THC_ERR_CUDA;
+  int st = static_init_current(device);
+  if (st != THC_OK) return st;
+  const StaticDev& d = g_static_dev[device];
+  const i64 tiles = ((M + 63) / 64) * ((N + 63) / 64), kiters = (K + 15) / 16;
+  if (tiles >= lim) return THC_ERR_OVERFLOW;
+  if (splits == 0) {
+    // about two waves of three 64 x 64 CTAs per SM, at least four k-tiles per split, within the scratch
+    const i64 want = std::max<i64>(1, (i64)d.sms * 6 / tiles);
+    splits = (int)std::max<i64>(1, std::min<i64>(std::min<i64>(want, kiters / 4), std::min<i64>(cap / per, 64)));
+  }
+  splits = (int)std::min<i64>(splits, kiters);              // no empty K ranges
+  if (splits > 65535) return THC_ERR_INVALID_ARG;           // grid.z
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+
+  thc::GemmParams p{};
+  p.A = A; p.B = B; p.aux = nullptr;
+  p.M = (int)M; p.N = (int)N; p.K = (int)K;
+  p.lda = lda; p.ldb = ldb;
+  p.batch = 1; p.kbatch = 1; p.splits = splits;
+  p.alpha = alpha; p.beta = beta;
+  if (splits > 1) { p.C = d.scratch; p.ldc = N; p.sCb = per; p.sCs = per; }
+  else            { p.C = C; p.ldc = ldc; }
+  const bool al16 = ((reinterpret_cast<uintptr_t>(A) | reinterpret_cast<uintptr_t>(B)) & 15) == 0 && (lda & 1) == 0 && (ldb & 1) == 0;
+  const int sm = thc::gemm_smem_bytes(64, 64, 16, 4, true, true);
+  const dim3 grid((unsigned)tiles, 1, (unsigned)splits);
+  if (al16) thc::dgemm_kernel<THC_SMALL, true, true, true><<<grid, thc::SMALL_THREADS, sm, s>>>(p);
+  else      thc::dgemm_kernel<THC_SMALL, true, true, false><<<grid, thc::SMALL_THREADS, sm, s>>>(p);
+  if (cudaPeekAtLastError() != cudaSuccess) { cudaGetLastError(); return THC_ERR_CUDA; }
+  if (splits > 1) {
+    thc::ReduceParams r{};
+    r.part = d.scratch; r.dst = C; r.aux = nullptr;
+    r.M = (int)M; r.N = (int)N; r.batch = 1; r.splits = splits;
+    r.ldd = ldc; r.alpha = alpha; r.beta = beta;
+    const int blocks = (int)std::max<i64>(1, std::min<i64>((per + 255) / 256, (i64)d.sms * 16));
+    thc::reduce_splits_kernel<<<blocks, 256, 0, s>>>(r);
+    if (cudaPeekAtLastError() != cudaSuccess) { cudaGetLastError(); return THC_ERR_CUDA; }
+  }
+  return THC_OK;
+}
