@@ -3,6 +3,7 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
                     [--bvv device|host|provider] [--trace FILE] [--probe] [--no-cpu-baseline]
+                    [--workload residual|second]
 
 One "step" = one pass of the whole hot path: thc_residual (R_PQ, all six terms)
 followed by thc_energy_device, on one seeded synthetic input set of BASELINE.json config C.  The default workload is
@@ -80,8 +81,11 @@ class OracleSample:
     configs 2-4 : the dense arrays do not fit host memory, so the oracle of record there is the sampled-row oracle
                   (oracle/rows.py).  The sample is one row R[P, :] of all six terms over the FIRST `nl` Cholesky vectors
                   (+ the xi intermediates and the energy over the same vectors); a whole evaluation is NP rows, and the
-                  Cholesky-dependent work (sigma1, sigma2, sigma3, xi, E) grows by NL / nl.  Both factors are stated in
-                  `sample`.
+                  Cholesky-dependent work (sigma1, sigma2, sigma3, xi, E) grows by NL / nl.  The sigma6 row, which alone
+                  takes minutes at config 3, is a sum over the ERI grid points I of identical pieces (THC ERIs expanded
+                  over (I, J), J always the whole grid): the sample evaluates it for the FIRST `nxi` points I (the oracle
+                  is handed the first nxi rows of V) and its time grows by NX / nxi.  All three factors are stated in
+                  `sample`; a step is a few seconds of CPU work.
     """
 
     def __init__(self, cfg, nl=None):
@@ -94,15 +98,24 @@ class OracleSample:
             self.sample = f"one full dense-oracle evaluation of config {cfg}"
         else:
             self.nl = nl or {2: 8, 3: 2, 4: 1}[cfg]
+            self.nxi = {2: 256, 3: 64, 4: 16}[cfg]
             self.x = make_inputs(c["o"], c["v"], c["NL"], c["NP"], c["NX"], c["seed"], l_keep=self.nl)
             self.kind = "rows"
             self.P = c["NP"] // 2
             self.sample = (f"sampled-row oracle (oracle/rows.py) on config {cfg}: one row P={self.P} of sigma1..sigma9, xi and E "
-                           f"over the first {self.nl} of {c['NL']} Cholesky vectors; a whole evaluation = NP={c['NP']} rows, "
-                           f"Cholesky-dependent parts x{c['NL'] / self.nl:.0f}")
+                           f"over the first {self.nl} of {c['NL']} Cholesky vectors, the sigma6 row over the first {self.nxi} of "
+                           f"{c['NX']} outer ERI-grid points; a whole evaluation = NP={c['NP']} rows, Cholesky-dependent parts "
+                           f"x{c['NL'] / self.nl:.0f}, sigma6 x{c['NX'] / self.nxi:.1f}")
 
     def run(self):
-        """Returns the estimated seconds of ONE whole oracle evaluation of the config."""
+        """Returns the estimated seconds of ONE whole oracle evaluation of the config; self.last_wall_s = what the
+        sample itself took."""
+        t_wall = time.perf_counter()
+        est = self._run()
+        self.last_wall_s = time.perf_counter() - t_wall
+        return est
+
+    def _run(self):
         import numpy as np
         x = self.x
         if self.kind == "dense":
@@ -122,10 +135,14 @@ class OracleSample:
         r = ro.row(self.P, terms=("s1", "s2", "s3"))
         t_lin = (time.perf_counter() - t0) * lscale                        # per row, all L
         t0 = time.perf_counter()
-        r.update(ro.row(self.P, terms=("s6", "s7", "s9")))
+        r.update(ro.row(self.P, terms=("s7", "s9")))
         t_quad = time.perf_counter() - t0                                  # per row, no L dependence
+        ro6 = RowOracle(x.Xo, x.Xv, x.Z, x.B_ov, x.B_oo, x.B_vv, x.Y, x.V[: self.nxi], x.eps, lblock=self.nl)
+        t0 = time.perf_counter()
+        r.update(ro6.row(self.P, terms=("s6",)))                           # outer grid points I < nxi only
+        t_s6 = (time.perf_counter() - t0) * c["NX"] / self.nxi
         assert all(np.isfinite(v).all() for v in r.values())
-        return t_once + c["NP"] * (t_lin + t_quad)
+        return t_once + c["NP"] * (t_lin + t_quad + t_s6)
 
 
 def time_oracle(cfg, budget_s=30.0):
@@ -147,12 +164,18 @@ def run_reference(args):
     s = OracleSample(args.config)
     for _ in range(args.warmup):
         s.run()
-    times = [s.run() for _ in range(args.steps)]
-    dt = sum(times) / len(times)
+    times, walls = [], []
+    for _ in range(args.steps):
+        times.append(s.run())
+        walls.append(s.last_wall_s)
+    dt = sum(times) / len(times)                     # seconds of one WHOLE evaluation (the sample's time scaled up)
     cores = len(os.sched_getaffinity(0))
     value = 1.0 / dt
+    # ms_per_step is what a step (= one bounded sample) really took, so that steps x ms_per_step is this run's timed region;
+    # `value` is whole evaluations per second, i.e. 1 / seconds_per_eval_extrapolated
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": 1e3 * sum(walls) / len(walls), "seconds_per_eval_extrapolated": dt,
+            "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"config{args.config}", "o": o, "v": v, "NL": NL, "NP": NP, "NX": NX},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
@@ -548,6 +571,78 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_second_workload(args):
+    """--workload second: the two appendix set-up steps at the dimensions of config C, timed with CUDA
+    events after 3 warm-ups, with the per-class split of the library's own launch timers.  mp2_density: thc_mp2_density on
+    (Xo, Xv, Z) of the config.  als_update: thc_cp_als_update on a projector-shaped array (U^P_ia), A[I = NP][J = o][K = v]
+    with N = NP factors and 10 PCG iterations.  Flop counts are those of the evaluation order in DESIGN.md section 6.8
+    (FMA = 2 flop, no padding).  One JSON line; not the BASELINE metric."""
+    import torch
+    import paper_2111_11473_b200 as thc
+    from thc_synth import CONFIGS
+    from thc_synth import device as synth
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --workload second: no CUDA device")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    c = CONFIGS[args.config]
+    o, v, NL, NP, NX = c["o"], c["v"], c["NL"], c["NP"], c["NX"]
+    K, W = max(1, args.steps), max(3, args.warmup)
+    pk = measured_peaks()
+    tensor_peak = pk["bf16"] * NOMINAL_FP64_TENSOR_OVER_BF16
+    h = thc.thc_setup(o, v, 4, NP, 16)
+    g = torch.Generator(device=dev).manual_seed(c["seed"])
+
+    def rnd(*shape, scale=1.0):
+        return torch.randn(*shape, dtype=torch.float64, device=dev, generator=g) * scale
+
+    def timed(fn):
+        for _ in range(W):
+            fn()
+        h.thc_profile_begin(7)
+        fn()
+        prof, work = h.thc_profile_end(), h.thc_profile_work()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = h.kernel_launches
+        a.record()
+        for _ in range(K):
+            fn()
+        b.record()
+        b.synchronize()
+        return a.elapsed_time(b) / K, prof, work, (h.kernel_launches - l0) // K
+
+    def report(ms, prof, work, launches, flops):
+        cls = {}
+        if prof["gemm"][0] > 0:
+            ach = work["gemm"] / (prof["gemm"][0] * 1e-3) / 1e12
+            cls["gemm"] = {"bound": "tensor", "ms": prof["gemm"][0], "launches": prof["gemm"][1], "achieved": ach,
+                           "peak": tensor_peak, "unit": "TFLOP/s", "frac": ach / tensor_peak}
+        if prof["ew"][0] > 0:
+            ach = work["ew"] / (prof["ew"][0] * 1e-3) / 1e9
+            cls["ew"] = {"bound": "hbm", "ms": prof["ew"][0], "launches": prof["ew"][1], "achieved": ach, "peak": pk["hbm"],
+                         "unit": "GB/s", "frac": ach / pk["hbm"]}
+        return {"ms": ms, "flops": flops, "tflops_fp64": flops / (ms * 1e-3) / 1e12, "gpu_launches": launches,
+                "executed_gemm_flops_over_counted": work["gemm"] / flops, "rooflines_by_class": cls}
+
+    Xo, Xv = rnd(o, NP, scale=NP ** -0.5), rnd(v, NP, scale=NP ** -0.5)
+    Z = rnd(NP, NP, scale=0.1)
+    Z = 0.5 * (Z + Z.T)
+    f_mp2 = (2.0 * NP * NP * (o + v) + 4.0 * NP ** 3 + 2.0 * (o + v) * NP * NP + 2.0 * (o * o + v * v) * NP
+             + 6.0 * o * v * NP * NP + 4.0 * o * NP ** 3 + 2.0 * o * NP * NP + 2.0 * o * o * NP + 2.0 * o * v * v * NP)
+    out = {"workload": "second (SURVEY.md 8(f)-4)", "config": {"workload": f"config{args.config} dimensions", "o": o, "v": v, "NP": NP},
+           "steps": K, "warmup": W, "dtype": "f64", "data": "synthetic"}
+    out["mp2_density"] = report(*timed(lambda: h.thc_mp2_density(Xo, Xv, Z)), f_mp2)
+    del Z
+    I, J, Kk, N, iters = NP, o, v, NP, 10
+    A = rnd(I, J, Kk)
+    Yf, Zf, Xf = rnd(J, N), rnd(Kk, N), rnd(I, N)
+    f_als = 2.0 * N * N * (J + Kk) + 2.0 * I * J * Kk * N + 2.0 * I * N * N * (iters + 1)
+    out["als_update"] = report(*timed(lambda: h.thc_cp_als_update(A, Yf, Zf, Xf, iters)), f_als)
+    out["als_update"]["shape"] = {"I": I, "J": J, "K": Kk, "N": N, "pcg_iters": iters}
+    h.close()
+    print(json.dumps(out), flush=True)
+
+
 def run_probe(args):
     """Measured ceilings of this device for the FP64 kernels (thc_probe in the library): DMMA and DFMA issue rates,
     both interleaved, shared-memory -> register bandwidth by access width."""
@@ -573,6 +668,8 @@ def main():
                     help="where B_vv lives (default: device; provider at config 4)")
     ap.add_argument("--trace", default=None, help="write the per-launch records of the profiled warm-up step to this CSV")
     ap.add_argument("--probe", action="store_true")
+    ap.add_argument("--workload", default="residual", choices=["residual", "second"],
+                    help="second = the appendix set-up steps (thc_mp2_density, thc_cp_als_update) at the config's dimensions")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the end-to-end (host buffers) leg")
     args = ap.parse_args()
@@ -580,6 +677,8 @@ def main():
         run_reference(args)
     elif args.probe:
         run_probe(args)
+    elif args.workload == "second":
+        run_second_workload(args)
     else:
         if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
             respawn_under_torchrun(args)

@@ -253,6 +253,32 @@ int thc_triple_product(thc_handle* h, int64_t nI, int64_t nPp, int64_t NPp, cons
  * clock in MHz, out[7] = 0. */
 int thc_probe(thc_handle* h, double out[8]);
 
+/* ---- second workload: the two O(N^4) set-up steps of PAPER.md's appendices, on the same kernels ----
+ *
+ * thc_mp2_density: MP2 one-particle density matrix from THC-factorised doubles, Appendix II (l.375-415):
+ *   D_oo[i][j] = -2 sum_kab t_ik^ab (2 t_jk^ab - t_jk^ba)   (Eq.47),   D_vv[a][b] = 2 sum_ijc t_ij^ac (2 t_ij^bc - t_ji^bc)   (Eq.48)
+ * with t_ij^ab = sum_PQ Xo[i,P] Xv[a,P] Z[P,Q] Xo[j,Q] Xv[b,Q] (Eq.23), evaluated in the O(N^4) factorisation of
+ * Eqs.51-56.  Xo [o][NP], Xv [v][NP], Z [NP][NP] (need not be symmetric), D_oo [o][o], D_vv [v][v]: device pointers,
+ * row-major, caller-owned; o, v, NP are the handle's.  Asynchronous on the handle's stream.  Needs
+ * thc_workspace_bytes_mp2 bytes of workspace (grown like thc_residual's when the library owns it, THC_ERR_NO_MEMORY when a
+ * caller-provided one is too small). */
+int64_t thc_workspace_bytes_mp2(const thc_handle* h);
+int thc_mp2_density(thc_handle* h, const double* Xo, const double* Xv, const double* Z, double* D_oo, double* D_vv);
+
+/* thc_cp_als_update: one alternating-least-squares factor update of a CP factorisation A_ijk ~ sum_n X_i^n Y_j^n Z_k^n
+ * (Appendix I, l.355-373): S of Eq.45, R of Eq.46, then `iters` iterations of the conjugate gradient method
+ * preconditioned with diag(S) on S x_i = R_i (Eq.44) for every row i, started from the X passed in (R22).
+ * A [I][J][K], Y [J][N], Z [K][N]: inputs; X [I][N]: in = starting guess, out = updated factor; rnorm2 [I] or NULL:
+ * |R_i - S x_i|^2 of the recurrence residual after the last iteration.  Device pointers, row-major, caller-owned;
+ * J * K < 2^31.  The sizes are independent of the handle's (it supplies device, stream and workspace:
+ * thc_workspace_bytes_als bytes).  The other two factors are updated by the same call on the permuted array (the paper
+ * keeps the three permutations of A resident, l.373).  Rows are independent (l.373): a multi-GPU update gives every
+ * rank a block of rows, A[i0:i1] and X[i0:i1], and the whole Y and Z -- no exchange inside the call, S is formed
+ * redundantly as in the paper; the caller gathers the updated rows.  Asynchronous. */
+int64_t thc_workspace_bytes_als(const thc_handle* h, int64_t I, int64_t J, int64_t K, int64_t N);
+int thc_cp_als_update(thc_handle* h, int64_t I, int64_t J, int64_t K, int64_t N, const double* A, const double* Y,
+                      const double* Z, double* X, int iters, double* rnorm2);
+
 /* ---- allocation-free entry point ------------------------------------------------------------------------------------
  * For callers that cannot call cudaMalloc (code under CUDA-graph capture, tight serving loops, harnesses that forbid
  * it): the split-K FP64 DMMA GEMM of the GEMM chains ("rate limiting step"; same kernels as thc_dgemm)

@@ -25,7 +25,8 @@ SYMBOLS = ("thc_setup", "thc_destroy", "thc_workspace_bytes", "thc_workspace_byt
            "thc_triple_product", "thc_strerror", "thc_last_cuda_error", "thc_last_error", "thc_shard_range",
            "thc_shard_doubles", "thc_residual_shard", "thc_residual_finish", "thc_energy_shard",
            "thc_profile_launches", "thc_profile_launch", "thc_algorithmic_work", "thc_probe", "thc_workspace_bytes_rr",
-           "thc_residual_rr", "thc_workspace_bytes_t1", "thc_residual_t1", "thc_static_init", "thc_dgemm_static")
+           "thc_residual_rr", "thc_workspace_bytes_t1", "thc_residual_t1", "thc_static_init", "thc_dgemm_static",
+           "thc_workspace_bytes_mp2", "thc_mp2_density", "thc_workspace_bytes_als", "thc_cp_als_update")
 
 STATIC_SCRATCH_BYTES = 16 << 20          # THC_STATIC_SCRATCH_BYTES of include/thc.h
 
@@ -136,6 +137,12 @@ def lib() -> ctypes.CDLL:
     L.thc_strerror.restype = ctypes.c_char_p
     L.thc_last_cuda_error.argtypes = [VP]
     L.thc_static_init.argtypes = [ctypes.c_int]
+    L.thc_workspace_bytes_mp2.argtypes = [VP]
+    L.thc_workspace_bytes_mp2.restype = I64
+    L.thc_mp2_density.argtypes = [VP, P, P, P, P, P]
+    L.thc_workspace_bytes_als.argtypes = [VP, I64, I64, I64, I64]
+    L.thc_workspace_bytes_als.restype = I64
+    L.thc_cp_als_update.argtypes = [VP, I64, I64, I64, I64, P, P, P, P, ctypes.c_int, P]
     L.thc_dgemm_static.argtypes = [ctypes.c_int, P, I64, I64, I64, ctypes.c_int, D, P, I64, P, I64, D, P, I64]
     for name in SYMBOLS:
         getattr(L, name)          # AttributeError if a declared symbol is missing
@@ -473,6 +480,34 @@ class Thc:
         _check(lib().thc_residual_host(self._h, *ptrs, _host_ptr(R_host, "R_host", self.NP * self.NP),
                                        ctypes.byref(E) if want_energy else None), self._h)
         return E.value if want_energy else None
+
+    def thc_mp2_density(self, Xo, Xv, Z):
+        """(D_oo [o, o], D_vv [v, v]) of PAPER.md Eqs.47-48 (App.II) for the THC amplitudes (Xo, Xv, Z)."""
+        import torch
+        need = lib().thc_workspace_bytes_mp2(self._h)
+        if need < 0:
+            _check(int(need), self._h)
+        self._prepare(max(self.workspace_bytes, need))
+        D_oo = torch.empty(self.o, self.o, dtype=torch.float64, device=self._device)
+        D_vv = torch.empty(self.v, self.v, dtype=torch.float64, device=self._device)
+        _check(lib().thc_mp2_density(self._h, _dev_ptr(Xo, "Xo", self.o * self.NP), _dev_ptr(Xv, "Xv", self.v * self.NP),
+                                     _dev_ptr(Z, "Z", self.NP * self.NP), _dev_ptr(D_oo, "D_oo"), _dev_ptr(D_vv, "D_vv")), self._h)
+        return D_oo, D_vv
+
+    def thc_cp_als_update(self, A, Y, Z, X, iters, want_rnorm2=False):
+        """One ALS update of the factor X [I, N] in place (App.I, Eqs.44-46; `iters` PCG iterations from X)."""
+        import torch
+        I, J, K = A.shape
+        N = X.shape[1]
+        need = lib().thc_workspace_bytes_als(self._h, I, J, K, N)
+        if need < 0:
+            _check(int(need), self._h)
+        self._prepare(max(self.workspace_bytes, need))
+        rn = torch.empty(I, dtype=torch.float64, device=self._device) if want_rnorm2 else None
+        _check(lib().thc_cp_als_update(self._h, I, J, K, N, _dev_ptr(A, "A", I * J * K), _dev_ptr(Y, "Y", J * N),
+                                       _dev_ptr(Z, "Z", K * N), _dev_ptr(X, "X", I * N), int(iters),
+                                       _dev_ptr(rn, "rnorm2") if want_rnorm2 else None), self._h)
+        return rn
 
     def thc_dgemm(self, a_kmajor, b_kmajor, M, N, K, alpha, A, lda, B, ldb, beta, C, ldc):
         # room for the split-K partial tiles of a skinny product (at most 64 splits of < 148 tiles)

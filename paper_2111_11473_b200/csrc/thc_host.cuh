@@ -454,6 +454,13 @@ struct Ctx {
     THC_EW(pair_accumulate_kernel, n * n, 8.0 * n * n * (n1 * n2 + 2.0), J, FA, ldfa, FB, ldfb, out, (int)n, (int)n1, (int)n2);
   }
   void diag(const double* A, double* d, i64 n) { THC_EW(diag_kernel, n, 16.0 * n, A, d, (int)n); }
+  // PCG over nrows independent systems (one warp per row)
+  void pcg_init(const double* r, const double* d, double* p, double* rz, i64 nrows, i64 n) {
+    THC_EW(pcg_init_kernel, nrows * 32, 8.0 * (2.0 * nrows * n + n + nrows), r, d, p, rz, (int)nrows, (int)n);
+  }
+  void pcg_iter(double* x, double* r, double* p, const double* Sp, const double* d, double* rz, i64 nrows, i64 n) {
+    THC_EW(pcg_iter_kernel, nrows * 32, 8.0 * (7.0 * nrows * n + n + 2.0 * nrows), x, r, p, Sp, d, rz, (int)nrows, (int)n);
+  }
   void copy(const double* src, double* dst, i64 n) {
     if (dry || !ok()) return;
     check(cudaMemcpyAsync(dst, src, (size_t)n * 8, cudaMemcpyDeviceToDevice, h->stream));

@@ -93,6 +93,61 @@ __global__ void diag_kernel(const double* __restrict__ A, double* __restrict__ d
   THC_GRID_STRIDE(idx, (i64)n) d[idx] = A[idx * n + idx];
 }
 
+// ---- preconditioned conjugate gradients on S x_i = R_i, one system per row i (App.I l.373: "solved on the GPU by
+// the preconditioned conjugate gradient method using the diagonal of S as the preconditioner"; the rows are independent).
+// One warp per row, lane j takes columns j, j + 32, ...; xor-shuffle reductions (fixed order: deterministic).
+__device__ __forceinline__ double warp_sum_all(double s) {
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+  return s;
+}
+// start: z = r / d, p = z, rz[i] = r_i . z_i      (r = R - X S was formed by a GEMM)
+__global__ void pcg_init_kernel(const double* __restrict__ r, const double* __restrict__ d, double* __restrict__ p,
+                                double* __restrict__ rz, int nrows, int n) {
+  const int lane = threadIdx.x & 31;
+  for (i64 row = ((i64)blockIdx.x * blockDim.x + threadIdx.x) >> 5; row < nrows; row += ((i64)gridDim.x * blockDim.x) >> 5) {
+    const double* rr = r + row * n;
+    double* pp = p + row * n;
+    double s = 0.0;
+    for (int c = lane; c < n; c += 32) {
+      const double z = rr[c] / d[c];
+      pp[c] = z;
+      s += rr[c] * z;
+    }
+    s = warp_sum_all(s);
+    if (lane == 0) rz[row] = s;
+  }
+}
+// one iteration given Sp = S p:  alpha = rz / p.Sp,  x += alpha p,  r -= alpha Sp,  z = r / d,  beta = r.z / rz,  p = z + beta p.
+// A row with p.Sp = 0 takes a zero step, a row with rz = 0 keeps beta = 0 (exactly converged rows stay put; oracle/als.py).
+__global__ void pcg_iter_kernel(double* __restrict__ x, double* __restrict__ r, double* __restrict__ p, const double* __restrict__ Sp,
+                                const double* __restrict__ d, double* __restrict__ rz, int nrows, int n) {
+  const int lane = threadIdx.x & 31;
+  for (i64 row = ((i64)blockIdx.x * blockDim.x + threadIdx.x) >> 5; row < nrows; row += ((i64)gridDim.x * blockDim.x) >> 5) {
+    double* xx = x + row * n;
+    double* rr = r + row * n;
+    double* pp = p + row * n;
+    const double* sp = Sp + row * n;
+    double pSp = 0.0;
+    for (int c = lane; c < n; c += 32) pSp += pp[c] * sp[c];
+    pSp = warp_sum_all(pSp);
+    const double rz_old = rz[row];
+    const double alpha = pSp != 0.0 ? rz_old / pSp : 0.0;
+    double rz_new = 0.0;
+    for (int c = lane; c < n; c += 32) {
+      xx[c] += alpha * pp[c];
+      const double rc = rr[c] - alpha * sp[c];
+      rr[c] = rc;
+      rz_new += rc * (rc / d[c]);
+    }
+    rz_new = warp_sum_all(rz_new);
+    const double beta = rz_old != 0.0 ? rz_new / rz_old : 0.0;
+    for (int c = lane; c < n; c += 32) pp[c] = rr[c] / d[c] + beta * pp[c];
+    __syncwarp();
+    if (lane == 0) rz[row] = rz_new;
+  }
+}
+
 // out[b*ldo + r] = sum_{i<n} X[r*ldx + i] * T[b*sTb + r*ldT + i]      (a^L_P: Alg.2 l.541, Alg.8 l.788; C7: Alg.7 line 9 l.749)
 // Eight lanes share a row (lane j takes i = j, j + 8, ...: 64-byte coalesced segments), xor-shuffle reduction.
 __global__ void rowdot_kernel(const double* __restrict__ X, i64 ldx, const double* __restrict__ T, i64 sTb, i64 ldT,

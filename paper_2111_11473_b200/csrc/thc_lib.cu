@@ -565,6 +565,88 @@ void plan_energy(Ctx& c, const double* Xo, const double* Xv, const double* Z, co
   c.final_sum(Eblk, nblk, 1.0, part2, nd, 2.0, E_dev, 0);
 }
 
+// ---- second workload ---------------------------------------------------------------------------------
+// MP2 one-particle density matrix from THC-factorised doubles, Appendix II (l.375-415): D_oo of Eq.47, D_vv of
+// Eq.48 in the O(N^4) factorisation of Eqs.51-56.  Coulomb-like parts (Eqs.53-54) are five NP^3 GEMMs and Hadamards.  The
+// exchange-like parts run over blocks of occupied orbitals i, every step one (batched) DMMA GEMM:
+//   Eq.55 as printed, innermost parenthesis first, with the Hadamards by o^{XZ} and the final v^{XY} sum as GEMM epilogues
+//   and a row-dot;
+//   Eq.56 with the o^{WZ} = sum_i y_i^W y_i^Z that closes its index cycle expanded last instead of first (the printed
+//   order forms a v x NP x NP intermediate per virtual a: v NP^3 flop; summing over i last shares M_i with Eq.55 and
+//   costs o NP^3):  D_ab -= 2 sum_i sum_X M_i[a][X] sum_Y o^{XY} (sum_Z y_i^Z v^{XZ} T^{YZ}) y_b^Y.
+void plan_mp2_density(Ctx& c, const double* Xo, const double* Xv, const double* Z, double* D_oo, double* D_vv) {
+  thc_handle* h = c.h;
+  thc::Arena& ar = c.ar;
+  const i64 o = h->o, v = h->v, NP = h->NP, NP2 = NP * NP, m0 = ar.mark();
+  double *omat = ar.alloc(NP2), *vmat = ar.alloc(NP2), *ovm = ar.alloc(NP2), *C1 = ar.alloc(NP2), *Km = ar.alloc(NP2);
+  double *tmpo = ar.alloc(o * NP), *tmpv = ar.alloc(v * NP);
+  c.gemm(Gemm(Xo, NP, 'M', Xo, NP, 'N', omat, NP, NP, NP, o));                    // Eq.51
+  c.gemm(Gemm(Xv, NP, 'M', Xv, NP, 'N', vmat, NP, NP, NP, v));                    // Eq.52
+  c.hadamard(omat, vmat, ovm, NP2);
+  c.gemm(Gemm(ovm, NP, 'K', Z, NP, 'K', C1, NP, NP, NP, NP));                     // sum_Z (o v)^{XZ} T^{YZ}
+  c.gemm(Gemm(Z, NP, 'K', C1, NP, 'N', Km, NP, NP, NP, NP));                      // K^{WY} = sum_X T^{WX} ( . )
+  c.hadamard(vmat, Km, C1, NP2);                                                  // Eq.53
+  c.gemm(Gemm(Xo, NP, 'K', C1, NP, 'N', tmpo, NP, o, NP, NP));
+  c.gemm(Gemm(tmpo, NP, 'K', Xo, NP, 'K', D_oo, o, o, o, NP).ab(-4.0, 0.0));
+  c.hadamard(omat, Km, C1, NP2);                                                  // Eq.54
+  c.gemm(Gemm(Xv, NP, 'K', C1, NP, 'N', tmpv, NP, v, NP, NP));
+  c.gemm(Gemm(tmpv, NP, 'K', Xv, NP, 'K', D_vv, v, v, v, NP).ab(4.0, 0.0));
+  const i64 per = 8 * (3 * v * NP + 2 * NP2 + NP);
+  const i64 bi = std::max<i64>(1, std::min<i64>(o, ((i64)256 << 20) / per));      // 256 MB of per-block intermediates
+  for (i64 i0 = 0; i0 < o; i0 += bi) {
+    const i64 ni = std::min<i64>(bi, o - i0), m1 = ar.mark();
+    double *Ai = ar.alloc(ni * v * NP), *Mi = ar.alloc(ni * v * NP), *Ni = ar.alloc(ni * NP2), *Ut = ar.alloc(ni * NP2);
+    double *w = ar.alloc(ni * NP), *Hb = ar.alloc(ni * NP * v);
+    c.rowscale(Xv, NP, Xo + i0 * NP, NP, nullptr, 1.0, Ai, ni, v, NP);                                        // y_i^W y_a^W
+    c.gemm(Gemm(Ai, NP, 'K', Z, NP, 'N', Mi, NP, ni * v, NP, NP));                                           // M_i[a][X] = sum_W T^{WX} ( . )
+    // Eq.55: N_i[Z][X] = o^{XZ} sum_a y_a^Z M_i[a][X];  Ut_i[Y][Z] = sum_X v^{XY} N_i[Z][X];  w_i[Y] = sum_Z T^{YZ} Ut_i[Y][Z]
+    c.gemm(Gemm(Xv, NP, 'M', Mi, NP, 'N', Ni, NP, NP, NP, v).batch(ni, 0, v * NP, NP2).aux(omat, NP, 0));
+    c.gemm(Gemm(vmat, NP, 'K', Ni, NP, 'K', Ut, NP, NP, NP, NP).batch(ni, 0, NP2, NP2));
+    c.rowdot(Z, NP, Ut, NP2, NP, w, NP, ni, NP, NP);
+    c.gemm(Gemm(w, NP, 'K', Xo, NP, 'K', D_oo + i0 * o, o, ni, o, NP).ab(2.0, 1.0));                          // sum_Y y_j^Y ( . )
+    // Eq.56: Vi[X][Z] = v^{XZ} y_i^Z;  G_i[X][Y] = o^{XY} sum_Z Vi[X][Z] T^{YZ};  H_i[X][b] = sum_Y G_i[X][Y] y_b^Y
+    c.rowscale(vmat, NP, Xo + i0 * NP, NP, nullptr, 1.0, Ni, ni, NP, NP);
+    c.gemm(Gemm(Ni, NP, 'K', Z, NP, 'K', Ut, NP, NP, NP, NP).batch(ni, NP2, 0, NP2).aux(omat, NP, 0));
+    c.gemm(Gemm(Ut, NP, 'K', Xv, NP, 'K', Hb, v, ni * NP, v, NP));
+    c.gemm(Gemm(Mi, NP, 'K', Hb, v, 'N', D_vv, v, v, v, NP).kbatch(ni, v * NP, NP * v).ab(-2.0, 1.0));        // sum_i sum_X M_i[a][X] H_i[X][b]
+    ar.release(m1);
+  }
+  ar.release(m0);
+}
+
+// One ALS factor update of a CP factorisation, Appendix I (l.355-373): S of Eq.45 (two Gram GEMMs, the Hadamard
+// product in the second one's epilogue), R of Eq.46 as ONE DMMA GEMM of the unfolded array with the Khatri-Rao product
+// KR[(j,k)][n] = Y_j^n Z_k^n, formed in blocks of j so that no array larger than the block is ever held (the paper
+// avoids the 3-index intermediate with a custom kernel; here the block is bounded and the flops run on the tensor
+// pipe), then `iters` PCG iterations on all rows at once: S p for every row is one GEMM, the rest of an iteration one
+// kernel with a warp per row.
+void plan_als_update(Ctx& c, i64 I, i64 J, i64 K, i64 N, const double* A, const double* Y, const double* Zf, double* X, int iters,
+                     double* rnorm2) {
+  thc::Arena& ar = c.ar;
+  const i64 m0 = ar.mark();
+  double *YtY = ar.alloc(N * N), *S = ar.alloc(N * N), *d = ar.alloc(N);
+  double *R = ar.alloc(I * N), *P = ar.alloc(I * N), *SP = ar.alloc(I * N), *rz = ar.alloc(I);
+  c.gemm(Gemm(Y, N, 'M', Y, N, 'N', YtY, N, N, N, J));
+  c.gemm(Gemm(Zf, N, 'M', Zf, N, 'N', S, N, N, N, K).aux(YtY, N, 0));                  // Eq.45
+  c.diag(S, d, N);
+  const i64 bj = std::max<i64>(1, std::min<i64>(J, ((i64)64 << 20) / (8 * K * N)));      // 64 MB Khatri-Rao blocks
+  for (i64 j0 = 0; j0 < J; j0 += bj) {
+    const i64 nj = std::min<i64>(bj, J - j0), m1 = ar.mark();
+    double* KR = ar.alloc(nj * K * N);
+    c.rowscale(Zf, N, Y + j0 * N, N, nullptr, 1.0, KR, nj, K, N);                      // KR[(j,k)][n] = Z_k^n Y_j^n
+    c.gemm(Gemm(A + j0 * K, J * K, 'K', KR, N, 'N', R, N, I, N, nj * K).ab(1.0, j0 ? 1.0 : 0.0));   // Eq.46
+    ar.release(m1);
+  }
+  c.gemm(Gemm(X, N, 'K', S, N, 'K', R, N, I, N, N).ab(-1.0, 1.0));                    // r = R - X S   (S symmetric)
+  c.pcg_init(R, d, P, rz, I, N);
+  for (int it = 0; it < iters; it++) {
+    c.gemm(Gemm(P, N, 'K', S, N, 'K', SP, N, I, N, N));
+    c.pcg_iter(X, R, P, SP, d, rz, I, N);
+  }
+  if (rnorm2) c.rowdot(R, N, R, 0, N, rnorm2, I, 1, I, N);
+  ar.release(m0);
+}
+
 // ---- dry runs: workspace sizes for the three entry points ------------------------------------------------------------
 struct Need { i64 arena_bytes, splitk_doubles; i64 total() const { return arena_bytes + (splitk_doubles * 8 + 255) / 256 * 256 + 256; } };
 
@@ -877,6 +959,19 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
     else if (!fix_bL && h->bL > 1) h->bL = h->bL / 2;
     else { delete h; return THC_ERR_NO_MEMORY; }
   }
+  // The work lists of Alg.6 line 11 for the row blocks of an unsharded evaluation (full block and tail) are uploaded
+  // here, so that the first evaluation neither allocates nor synchronises; other shapes (shards) are built on first use.
+  if (h->t2sq_algorithm != 5 && (h->term_mask == 0 || (h->term_mask & THC_TERM_S6))) {
+    DeviceGuard g(dev);
+    Ctx c{h};
+    c.dry = false;
+    const i64 NPp = pad_to(NP, thc::TP_RT), full = std::min<i64>(h->bX, NP), tail = NP % full;
+    if (g.ok) {
+      c.triple_items(pad_to(full, thc::TP_PT), NPp);
+      if (tail) c.triple_items(pad_to(tail, thc::TP_PT), NPp);
+    }
+    if (!g.ok || c.status != THC_OK) { const int st = g.ok ? c.status : THC_ERR_CUDA; thc_destroy(h); return st; }
+  }
   *hp = h;
   return THC_OK;
 }
@@ -1133,6 +1228,65 @@ int thc_energy_shard(thc_handle* h, const double* Xo, const double* Xv, const do
   st = ensure_workspace(h, h->need_bytes);
   if (st != THC_OK) return st;
   return run_energy(h, static_cast<char*>(h->ws), h->ws_bytes, Xo, Xv, Z, B_ov, nullptr, E_dev, r[1] - r[0]);
+}
+
+// ---- second workload ---------------------------------------------------------------------------------
+static Need dry_mp2(thc_handle* h) {
+  Ctx c{h}; c.dry = true; c.ar.dry = true;
+  plan_mp2_density(c, nullptr, nullptr, nullptr, nullptr, nullptr);
+  return Need{c.ar.peak, c.splitk_need};
+}
+static Need dry_als(thc_handle* h, i64 I, i64 J, i64 K, i64 N) {
+  Ctx c{h}; c.dry = true; c.ar.dry = true;
+  plan_als_update(c, I, J, K, N, nullptr, nullptr, nullptr, nullptr, 1, reinterpret_cast<double*>(static_cast<uintptr_t>(256)));
+  return Need{c.ar.peak, c.splitk_need};
+}
+
+int64_t thc_workspace_bytes_mp2(const thc_handle* h) {
+  return h ? dry_mp2(const_cast<thc_handle*>(h)).total() : (int64_t)THC_ERR_INVALID_ARG;
+}
+
+int thc_mp2_density(thc_handle* h, const double* Xo, const double* Xv, const double* Z, double* D_oo, double* D_vv) {
+  if (!h || bad_ptr(Xo) || bad_ptr(Xv) || bad_ptr(Z) || bad_ptr(D_oo) || bad_ptr(D_vv)) return THC_ERR_INVALID_ARG;
+  DeviceGuard g(h->device);
+  if (!g.ok) return THC_ERR_CUDA;
+  const Need need = dry_mp2(h);
+  int st = ensure_workspace(h, std::max<i64>(h->need_bytes, need.total()));
+  if (st != THC_OK) return st;
+  Ctx c{h};
+  st = make_ctx(c, h, static_cast<char*>(h->ws), h->ws_bytes, need);
+  if (st != THC_OK) return st;
+  plan_mp2_density(c, Xo, Xv, Z, D_oo, D_vv);
+  if (c.ar.overflow) return THC_ERR_NO_MEMORY;
+  return c.status;
+}
+
+static bool als_dims_ok(int64_t I, int64_t J, int64_t K, int64_t N) {
+  const int64_t lim = (int64_t)1 << 31;
+  return I > 0 && J > 0 && K > 0 && N > 0 && I < lim && N < lim && J < lim && K < lim && (long double)J * K < (long double)lim &&
+         (long double)I * J * K * 8 < 9e18L;
+}
+
+int64_t thc_workspace_bytes_als(const thc_handle* h, int64_t I, int64_t J, int64_t K, int64_t N) {
+  if (!h || !als_dims_ok(I, J, K, N)) return (int64_t)THC_ERR_INVALID_ARG;
+  return dry_als(const_cast<thc_handle*>(h), I, J, K, N).total();
+}
+
+int thc_cp_als_update(thc_handle* h, int64_t I, int64_t J, int64_t K, int64_t N, const double* A, const double* Y,
+                      const double* Z, double* X, int iters, double* rnorm2) {
+  if (!h || !als_dims_ok(I, J, K, N) || iters < 0) return THC_ERR_INVALID_ARG;
+  if (bad_ptr(A) || bad_ptr(Y) || bad_ptr(Z) || bad_ptr(X) || (rnorm2 && bad_ptr(rnorm2))) return THC_ERR_INVALID_ARG;
+  DeviceGuard g(h->device);
+  if (!g.ok) return THC_ERR_CUDA;
+  const Need need = dry_als(h, I, J, K, N);
+  int st = ensure_workspace(h, std::max<i64>(h->need_bytes, need.total()));
+  if (st != THC_OK) return st;
+  Ctx c{h};
+  st = make_ctx(c, h, static_cast<char*>(h->ws), h->ws_bytes, need);
+  if (st != THC_OK) return st;
+  plan_als_update(c, I, J, K, N, A, Y, Z, X, iters, rnorm2);
+  if (c.ar.overflow) return THC_ERR_NO_MEMORY;
+  return c.status;
 }
 
 int thc_profile_begin(thc_handle* h, int class_mask) {

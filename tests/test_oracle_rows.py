@@ -53,3 +53,17 @@ def test_single_xi_column_and_row_match_dense(dims):
         assert np.abs(ro.xi_oo_column(j) - ref["xi_oo"][:, j]).max() <= 1e-12 * np.abs(ref["xi_oo"]).max(), j
     for b in range(x.v):
         assert np.abs(ro.xi_vv_row(b) - ref["xi_vv"][b]).max() <= 1e-12 * np.abs(ref["xi_vv"]).max(), b
+
+
+def test_sigma6_row_over_the_first_outer_grid_points():
+    """bench.py's bounded CPU sample hands the row oracle the first nxi rows of V: the sigma6 row is then the partial sum
+    over the outer ERI-grid points I < nxi (J over the whole grid), i.e. the full row for a V whose other rows are zero."""
+    x = small_inputs(3, 4, 5, 6, 10, seed=12)
+    nxi, P = 4, 2
+    part = RowOracle(x.Xo, x.Xv, x.Z, x.B_ov, x.B_oo, x.B_vv, x.Y, x.V[:nxi], x.eps).row(P, terms=("s6",))["s6"]
+    Vz = x.V.copy()
+    Vz[nxi:] = 0.0
+    full = RowOracle(x.Xo, x.Xv, x.Z, x.B_ov, x.B_oo, x.B_vv, x.Y, Vz, x.eps).row(P, terms=("s6",))["s6"]
+    assert np.abs(part - full).max() <= 1e-14 * np.abs(full).max()
+    whole = RowOracle(x.Xo, x.Xv, x.Z, x.B_ov, x.B_oo, x.B_vv, x.Y, x.V, x.eps).row(P, terms=("s6",))["s6"]
+    assert np.abs(part - whole).max() > 1e-3 * np.abs(whole).max()          # it really is a part, not the whole
