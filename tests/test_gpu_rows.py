@@ -1,7 +1,8 @@
 """Parity of the CUDA path against the T2 sampled-row oracle (oracle/rows.py) at sizes the dense oracle cannot hold.
 
 Configs 2 and 3 run by default, in the launch configuration bench.py times (config 3 is its default workload); config 4
-is opt-in (THC_BIG_TESTS=4: an evaluation takes ~13 minutes and the CPU rows about an hour).  Inputs are drawn on the device by
+is opt-in (THC_BIG_TESTS=4: an evaluation takes ~13 minutes; its oracle rows take hours of CPU and are read from
+tests/golden/ where tests/golden/make_rows.py has stored them, else computed live).  Inputs are drawn on the device by
 thc_synth.device and the very same tensors are copied to the host for the oracle.  Tolerances as in test_gpu_parity.py:
 1e-10 relative to each term's own maximum over the sampled rows, 1e-9 E_h on the energy.
 """
@@ -89,16 +90,28 @@ def _run(cfg, rows, rows_s6, lblock, terms=TERMS, check_xi_and_energy=True, prov
         s9_ref = RowOracle(*zero, lblock=1).row(cheap_pins["P"], terms=("s9",))["s9"]
         errs["s9_eps_part"] = np.abs(cheap["s9_eps"] - s9_ref).max() / np.abs(s9_ref).max()
         print(f"config {cfg}: cheap pins (E per vector, xi column/row, sigma9 eps part) {time.perf_counter() - t0:.0f} s CPU", flush=True)
+    # stored expected rows (tests/golden/config<C>_row<P>_<term>.txt, written by tests/golden/make_rows.py from oracle/ alone)
+    # replace the live oracle for the terms they hold: at config 4 a row takes longer than a GPU-box call may last
+    from golden.make_rows import load_rows
+    stored = {P: load_rows(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden"), cfg, P) for P in rows}
+    if any("s6" in stored[P] for P in rows) and "s6" not in terms:
+        terms = tuple(k for k in TERMS if k in terms or k == "s6")
     ref = {k: [] for k in terms}
     all_terms = terms
     for n, P in enumerate(rows):
-        terms = all_terms if P in rows_s6 else tuple(k for k in all_terms if k != "s6")
+        terms = tuple(k for k in all_terms if k != "s6" or P in rows_s6 or "s6" in stored[P])
+        live = tuple(k for k in terms if k not in stored[P])
         t0 = time.perf_counter()
-        r = ro.row(P, terms=terms)
-        print(f"config {cfg}: oracle row P={P} terms {terms}: {time.perf_counter() - t0:.0f} s CPU", flush=True)
+        r = dict(stored[P])
+        if live:
+            r.update(ro.row(P, terms=live))
+        print(f"config {cfg}: oracle row P={P}: live {live} in {time.perf_counter() - t0:.0f} s CPU, stored "
+              f"{tuple(k for k in terms if k in stored[P])}", flush=True)
         for k in terms:
             ref[k].append((n, r[k]))
     for k in all_terms:
+        if not ref[k]:
+            continue
         scale = max(np.abs(r).max() for _, r in ref[k])
         errs[k] = max(np.abs(got[k][n] - r).max() for n, r in ref[k]) / scale
     bad = {k: e for k, e in errs.items() if e > (1e-9 if k.startswith("E_") else 1e-10)}
@@ -116,8 +129,8 @@ def test_config3_sampled_rows():
 
 
 @pytest.mark.skipif(not os.environ.get("THC_BIG_TESTS", "").startswith("4"),
-                    reason="set THC_BIG_TESTS=4 (config 4: ~40 GB resident, B_vv streamed, ~15 min of GPU and ~1 h of CPU "
-                           "row oracle; THC_BIG_TESTS=4s6 adds one row of sigma6, ~40 min more)")
+                    reason="set THC_BIG_TESTS=4 (config 4: ~40 GB resident, B_vv streamed, ~15 min of GPU; rows stored under "
+                           "tests/golden/ are used, missing ones cost ~1 h of CPU; THC_BIG_TESTS=4s6 forces a sigma6 row)")
 def test_config4_sampled_rows_streamed_bvv():
     """Paper-scale config: B_vv (304 GB) comes from a provider callback one L-block at a time.  One sampled row of
     sigma1, sigma2, sigma3, sigma7 (and sigma6 with THC_BIG_TESTS=4s6) against the row oracle; the energy through

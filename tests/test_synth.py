@@ -1,4 +1,6 @@
 """The seeded input generator: determinism, order-freedom, structure (no method arithmetic in it)."""
+import os
+
 import numpy as np
 
 from thc_synth import make_inputs, bvv_block, normal_block, CONFIGS
@@ -57,3 +59,33 @@ def test_device_generator_matches_numpy_generator():
         assert np.abs(getattr(x, k) - d[k].numpy()).max() <= 1e-14, k
     blk = dv.bvv_block(9, 3, 4, 6, 2, 5, "cpu").numpy()
     assert np.abs(blk - x.B_vv[2:5]).max() <= 1e-14
+
+
+def test_lazy_cholesky_blocks_equal_the_full_arrays():
+    """LazyCholesky draws B_oo / B_ov block by block: any slice equals the same slice of the arrays make_inputs returns."""
+    from thc_synth import LazyCholesky, make_inputs
+    x = make_inputs(3, 5, 9, 4, 6, seed=11, with_bvv=False)
+    for kind, full in (("oo", x.B_oo), ("ov", x.B_ov)):
+        lazy = LazyCholesky(11, 3, 5, 9, kind)
+        assert lazy.shape == full.shape
+        for sl in (slice(0, 4), slice(4, 9), slice(8, 12)):
+            assert np.array_equal(lazy[sl], full[sl])
+
+
+def test_golden_row_writer_round_trip(tmp_path):
+    """tests/golden/make_rows.py (oracle + generators only) writes exact hex floats; drawing the Cholesky vectors block by
+    block gives the rows of the in-memory oracle up to the summation order over L-blocks."""
+    import subprocess
+    import sys
+    from golden.make_rows import load_rows
+    from oracle.rows import RowOracle
+    from thc_synth import make_config
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    subprocess.run([sys.executable, os.path.join(root, "tests", "golden", "make_rows.py"), "--config", "0", "--row", "7",
+                    "--terms", "s1,s2,s3,s6,s7", "--outdir", str(tmp_path)], check=True, timeout=600, cwd=root)
+    got = load_rows(str(tmp_path), 0, 7)
+    x = make_config(0)
+    ref = RowOracle(x.Xo, x.Xv, x.Z, x.B_ov, x.B_oo, x.B_vv, x.Y, x.V, x.eps).row(7, terms=tuple(got))
+    assert set(got) == {"s1", "s2", "s3", "s6", "s7"}
+    for k in got:
+        assert np.abs(got[k] - ref[k]).max() <= 1e-13 * np.abs(ref[k]).max(), k

@@ -5,7 +5,7 @@ tensors (BASELINE.json `configs`; recipe restated in DESIGN.md section 4).  It i
 the one module both the CPU oracle tests and the CUDA path tests may import.
 """
 from .generators import (CONFIGS, ThcInputs, make_inputs, make_config, config_dims,
-                         normal_block, uniform_block, bvv_block, TENSOR_IDS)
+                         normal_block, uniform_block, bvv_block, TENSOR_IDS, LazyCholesky)
 
 __all__ = ["CONFIGS", "ThcInputs", "make_inputs", "make_config", "config_dims",
-           "normal_block", "uniform_block", "bvv_block", "TENSOR_IDS"]
+           "normal_block", "uniform_block", "bvv_block", "TENSOR_IDS", "LazyCholesky"]

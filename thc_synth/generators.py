@@ -108,6 +108,24 @@ def bvv_block(seed: int, o: int, v: int, NL: int, L0: int, L1: int) -> np.ndarra
     return _bsym_block(seed, o + v, NL, L0, L1, o, o + v, o, o + v)
 
 
+class LazyCholesky:
+    """B_oo ("oo") or B_ov ("ov") of a workload as an array-like that draws the requested Cholesky vectors on demand:
+    `.shape` and `[L0:L1]` only (what an L-blocked consumer needs).  At config 4 B_ov alone is 34 GB; a consumer that
+    walks the vectors block by block never has to hold it."""
+
+    def __init__(self, seed, o, v, NL, kind):
+        self.seed, self.o, self.v, self.NL, self.kind = seed, o, v, NL, kind
+        self.shape = (NL, o, o if kind == "oo" else v)
+
+    def __getitem__(self, key):
+        if not isinstance(key, slice) or key.step not in (None, 1):
+            raise IndexError("LazyCholesky supports contiguous slices of the Cholesky index only")
+        L0, L1, _ = key.indices(self.NL)
+        o, n = self.o, self.o + self.v
+        q0, q1 = (0, o) if self.kind == "oo" else (o, n)
+        return np.ascontiguousarray(_bsym_block(self.seed, n, self.NL, L0, L1, 0, o, q0, q1))
+
+
 @dataclass
 class ThcInputs:
     o: int
