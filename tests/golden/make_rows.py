@@ -48,6 +48,9 @@ def main():
     ap.add_argument("--row", type=int, required=True)
     ap.add_argument("--terms", required=True, help="comma-separated subset of s1,s2,s3,s6,s7 (sigma9 needs the full xi)")
     ap.add_argument("--lblock", type=int, default=4)
+    ap.add_argument("--bvv-on-gpu", action="store_true",
+                    help="draw the B_vv blocks with thc_synth.device on cuda:0 (same seeded function, values equal to an ulp or "
+                         "two); the numpy generator needs ~1 s per vector at config 4, i.e. hours per row")
     ap.add_argument("--outdir", default=os.path.dirname(os.path.abspath(__file__)))
     args = ap.parse_args()
     terms = tuple(args.terms.split(","))
@@ -60,6 +63,9 @@ def main():
     if any(t in LINEAR_IN_B for t in terms):                                  # the Cholesky vectors, drawn block by block
         B_ov, B_oo = LazyCholesky(seed, o, v, NL, "ov"), LazyCholesky(seed, o, v, NL, "oo")
         B_vv = lambda L0, L1: bvv_block(seed, o, v, NL, L0, L1)
+        if args.bvv_on_gpu:
+            from thc_synth import device as synth
+            B_vv = lambda L0, L1: synth.bvv_block(seed, o, v, NL, L0, L1, "cuda").cpu().numpy()
     else:
         B_ov, B_oo, B_vv = x.B_ov, x.B_oo, np.zeros((1, v, v))
     print(f"inputs drawn in {time.perf_counter() - t0:.0f} s", flush=True)
@@ -71,7 +77,8 @@ def main():
         path = row_file(args.outdir, args.config, args.row, term)
         with open(path, "w") as f:
             f.write(f"# R[P={args.row}, :] of term {term}, BASELINE config {args.config} (o={o} v={v} NL={NL} NP={NP} NX={NX}, seed {seed})\n")
-            f.write(f"# written by tests/golden/make_rows.py from oracle/rows.py (RowOracle.row, lblock={args.lblock}) in {dt:.0f} s CPU, "
+            f.write(f"# written by tests/golden/make_rows.py from oracle/rows.py (RowOracle.row, lblock={args.lblock}"
+                    f"{', B_vv blocks drawn by thc_synth.device' if args.bvv_on_gpu and term in ('s1', 's3') else ''}) in {dt:.0f} s CPU, "
                     f"{time.strftime('%Y-%m-%d')}; C99 hex floats\n")
             for k in range(0, NP, 4):
                 f.write(" ".join(float(val).hex() for val in row[k:k + 4]) + "\n")
