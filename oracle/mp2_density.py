@@ -30,3 +30,26 @@ def density_from_amplitudes(t):
 def mp2_density(Xo, Xv, Z):
     """(D_oo, D_vv) for the THC amplitudes of Eq.23 (Eqs.49-50 l.387-391 are Eqs.47-48 with Eq.23 inserted)."""
     return density_from_amplitudes(dense.expand_t(Xo, Xv, Z))
+
+
+# ---- single elements, for shapes whose dense t (o^2 v^2 doubles) does not fit ----------------------------------------------
+def _t_fixed_i(Xo, Xv, Z, i):
+    """t[a, k, b] = t_ik^ab for one occupied index i (Eq.23)."""
+    return np.einsum("aP,PQ,kQ,bQ->akb", Xv * Xo[i], Z, Xo, Xv, optimize=True)
+
+
+def _t_fixed_a(Xo, Xv, Z, a):
+    """t[i, j, c] = t_ij^ac for one virtual index a (Eq.23)."""
+    return np.einsum("iP,PQ,jQ,cQ->ijc", Xo * Xv[a], Z, Xo, Xv, optimize=True)
+
+
+def density_oo_element(Xo, Xv, Z, i, j):
+    """D_ij of Eq.47 alone: -2 sum_kab t_ik^ab (2 t_jk^ab - t_jk^ba)."""
+    ti, tj = _t_fixed_i(Xo, Xv, Z, i), _t_fixed_i(Xo, Xv, Z, j)
+    return -2.0 * (2.0 * np.sum(ti * tj) - np.einsum("akb,bka->", ti, tj))
+
+
+def density_vv_element(Xo, Xv, Z, a, b):
+    """D_ab of Eq.48 alone: 2 sum_ijc t_ij^ac (2 t_ij^bc - t_ji^bc)."""
+    ta, tb = _t_fixed_a(Xo, Xv, Z, a), _t_fixed_a(Xo, Xv, Z, b)
+    return 2.0 * (2.0 * np.sum(ta * tb) - np.einsum("ijc,jic->", ta, tb))

@@ -110,3 +110,28 @@ def test_row_blocks_are_independent():
     finally:
         h.close()
     assert np.abs(got - want).max() <= 1e-12 * np.abs(want).max()
+
+
+def test_als_update_at_config2_size_sampled_rows():
+    """Projector-shaped array at BASELINE config 2 dimensions (I = NP = 1000, J = o = 60, K = v = 340, N = 1000 factors): the
+    rows of the update are independent, so the oracle is run on three sampled rows (with the whole Y, Z)."""
+    import torch
+    import paper_2111_11473_b200 as thc
+    from oracle import als
+    I, J, K, N, iters = 1000, 60, 340, 1000, 8
+    g = torch.Generator(device="cuda").manual_seed(5)
+    rnd = lambda *s: torch.randn(*s, dtype=torch.float64, device="cuda", generator=g)
+    A, Y, Z, X = rnd(I, J, K), rnd(J, N), rnd(K, N), rnd(I, N)
+    rows = [0, 517, 999]
+    X0 = X[rows].cpu().numpy()
+    h = thc.thc_setup(2, 3, 2, 8, 8)
+    try:
+        rn = h.thc_cp_als_update(A, Y, Z, X, iters, want_rnorm2=True)
+        torch.cuda.synchronize()
+    finally:
+        h.close()
+    want, want_rn = als.als_update(A[rows].cpu().numpy(), Y.cpu().numpy(), Z.cpu().numpy(), X0, iters)
+    got = X[rows].cpu().numpy()
+    assert np.abs(got - want).max() <= TOL * np.abs(want).max(), np.abs(got - want).max() / np.abs(want).max()
+    scale = np.sum(als.mttkrp(A[rows].cpu().numpy(), Y.cpu().numpy(), Z.cpu().numpy()) ** 2, axis=1).max()
+    assert np.abs(rn[rows].cpu().numpy() - want_rn).max() <= TOL * scale

@@ -44,3 +44,28 @@ def test_mp2_density_with_a_non_symmetric_core_matrix():
 def test_mp2_density_over_several_blocks_of_occupied_orbitals():
     """o NP^2 large enough that the exchange-like parts run in two blocks of i with a ragged last one (22 + 2)."""
     _run(24, 60, 800, seed=9)
+
+
+def test_mp2_density_at_config2_size_sampled_elements_and_invariants():
+    """BASELINE config 2 dimensions (o=60, v=340, NP=1000): the dense t does not fit the oracle, so single elements of
+    D_oo / D_vv from their definition (oracle.mp2_density.density_*_element) plus what holds at any size: symmetry and
+    tr D_oo = -tr D_vv."""
+    import torch
+    import paper_2111_11473_b200 as thc
+    from thc_synth import make_inputs
+    from oracle import mp2_density
+    o, v, NP = 60, 340, 1000
+    x = make_inputs(o, v, 4, NP, 8, seed=2, with_bvv=False)
+    Z = x.Z * 30.0
+    h = thc.thc_setup(o, v, 4, NP, 8)
+    try:
+        D_oo, D_vv = (t.cpu().numpy() for t in h.thc_mp2_density(*[torch.from_numpy(np.ascontiguousarray(t)).cuda() for t in (x.Xo, x.Xv, Z)]))
+    finally:
+        h.close()
+    so, sv = np.abs(D_oo).max(), np.abs(D_vv).max()
+    for i, j in ((3, 7), (59, 59)):
+        assert abs(D_oo[i, j] - mp2_density.density_oo_element(x.Xo, x.Xv, Z, i, j)) <= TOL * so, (i, j)
+    for a, b in ((5, 123), (339, 339)):
+        assert abs(D_vv[a, b] - mp2_density.density_vv_element(x.Xo, x.Xv, Z, a, b)) <= TOL * sv, (a, b)
+    assert np.abs(D_oo - D_oo.T).max() <= 1e-12 * so and np.abs(D_vv - D_vv.T).max() <= 1e-12 * sv
+    assert abs(np.trace(D_oo) + np.trace(D_vv)) <= 1e-11 * abs(np.trace(D_vv))

@@ -95,3 +95,16 @@ def test_factorised_eqs_53_56_reproduce_the_definition():
         got_oo, got_vv = _eqs_53_56(Xo, Xv, Z)
         assert np.abs(got_oo - want_oo).max() <= 1e-12 * np.abs(want_oo).max()
         assert np.abs(got_vv - want_vv).max() <= 1e-12 * np.abs(want_vv).max()
+
+
+def test_single_elements_equal_the_dense_blocks():
+    """density_oo_element / density_vv_element (used at sizes where the dense t does not fit) against the dense oracle,
+    every element, with a non-symmetric Z so that the index positions of the exchange parts matter."""
+    Xo, Xv, Z = _problem(3, 4, 5, seed=29, symmetric=False)
+    D_oo, D_vv = mp2_density.mp2_density(Xo, Xv, Z)
+    for i in range(3):
+        for j in range(3):
+            assert abs(mp2_density.density_oo_element(Xo, Xv, Z, i, j) - D_oo[i, j]) <= 1e-12 * np.abs(D_oo).max()
+    for a in range(4):
+        for b in range(4):
+            assert abs(mp2_density.density_vv_element(Xo, Xv, Z, a, b) - D_vv[a, b]) <= 1e-12 * np.abs(D_vv).max()
