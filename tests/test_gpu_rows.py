@@ -57,6 +57,8 @@ def _run(cfg, rows, rows_s6, lblock, terms=TERMS, check_xi_and_energy=True, prov
         h0.close()
         del r0
     got = {k: res[k][list(rows)].cpu().numpy() for k in TERMS + ("R",)}
+    if os.environ.get("THC_ROWS_SAVE"):          # the sampled GPU rows, for tests/test_rows_offline.py (stored oracle rows that
+        np.savez(os.environ["THC_ROWS_SAVE"], cfg=cfg, rows=np.array(rows), **got)      # arrive after this run)
     xi_oo, xi_vv = res["xi_oo"].cpu().numpy(), res["xi_vv"].cpu().numpy()
     sym = float((res["R"] - res["R"].T).abs().max() / res["R"].abs().max())
     h.close()
