@@ -37,6 +37,7 @@ struct thc_handle {
   // Alg.6 line 11: work-item lists (device memory owned by the handle), one per (nPp, NPp) shape seen
   struct TripleList { int64_t nPp, NPp; thc::TripleItem* dev; int n; };
   std::vector<TripleList> tp_lists;
+  bool tp_gate = true;               // gate the long line-11 launches; cleared for good if a cooperative launch is refused
   void* encode_tiled;                // cuTensorMapEncodeTiled, resolved through the runtime (no -lcuda link)
   // B_vv streaming (THC_BVV_HOST): copy stream and double-buffer events, created on first use
   int bvv_mode;
@@ -601,7 +602,8 @@ struct Ctx {
               for (int qb = qb0; qb < std::min(qb0 + 6, nqb); qb++)
                 if (qb <= 2 * rb + 1) items.push_back(TripleItem{pt * TP_PT, qb * TP_QT, rb * TP_RT, (qb >> 1) == rb ? 1 : 0});
     thc_handle::TripleList l{nPp, NPp, nullptr, (int)items.size()};
-    if (cudaMalloc(&l.dev, items.size() * sizeof(TripleItem)) != cudaSuccess) { check(cudaGetLastError()); return nullptr; }
+    // (+ 4 slots: the gate counter of the launches that use this list lives behind the items)
+    if (cudaMalloc(&l.dev, (items.size() + 4) * sizeof(TripleItem)) != cudaSuccess) { check(cudaGetLastError()); return nullptr; }
     // pageable source: the runtime stages the data before returning, so `items` may die at the end of this scope
     check(cudaMemcpyAsync(l.dev, items.data(), items.size() * sizeof(TripleItem), cudaMemcpyHostToDevice, h->stream));
     check(cudaStreamSynchronize(h->stream));
@@ -622,8 +624,23 @@ struct Ctx {
     p.nI = (int)nI; p.nPp = (int)nPp; p.NPp = (int)NPp; p.accumulate = accumulate;
     const int grid = std::min(list->n, h->sms);
     if (((i64)(list->n + grid - 1) / grid) * nI >= ((i64)1 << 31)) { status = THC_ERR_OVERFLOW; return; }
+    // Long launches (>= 32 items per CTA) run gated: a cooperative launch (all CTAs co-resident) in which the CTAs wait
+    // for one another every ~2048 grid points of work, so that the L2-ordered work list keeps paying (thc_triple.cuh).
+    p.gate = reinterpret_cast<unsigned int*>(list->dev + list->n);
+    p.gate_every = (h->tp_gate && list->n >= 32 * grid) ? (int)std::max<i64>(1, std::min<i64>(32, 2048 / std::max<i64>(1, nI))) : 0;
     prof_start(1, "triple_product", 5.0 * nI * nPp * (double)NPp * NPp);
-    triple_product_kernel<<<grid, TP_THREADS, TP_SMEM_BYTES, h->stream>>>(mE, mF, mG, p);
+    if (p.gate_every) {
+      check(cudaMemsetAsync(p.gate, 0, sizeof(unsigned int), h->stream));
+      void* args[4] = {&mE, &mF, &mG, &p};
+      cudaError_t e = cudaLaunchCooperativeKernel(reinterpret_cast<void*>(triple_product_kernel), dim3(grid), dim3(TP_THREADS), args,
+                                                  TP_SMEM_BYTES, h->stream);
+      if (e != cudaSuccess) {              // not launchable that way here: never gate again on this handle
+        cudaGetLastError();
+        h->tp_gate = false;
+        p.gate_every = 0;
+      }
+    }
+    if (!p.gate_every) triple_product_kernel<<<grid, TP_THREADS, TP_SMEM_BYTES, h->stream>>>(mE, mF, mG, p);
     launched();
     prof_stop(1);
   }

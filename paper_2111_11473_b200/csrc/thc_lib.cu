@@ -879,6 +879,7 @@ int thc_setup(thc_handle** hp, int64_t o, int64_t v, int64_t NL, int64_t NP, int
     h->t2sq_algorithm = want ? want : ((t5 < t4 && n5_fits) ? 5 : 4);
   }
   h->prof_mask = 0; h->prof_used = 0; h->prof_done = 0; h->encode_tiled = nullptr;
+  h->tp_gate = true;
   h->cap_stream = nullptr;
   {
     const int ug = opt ? opt->use_graph : -1;
