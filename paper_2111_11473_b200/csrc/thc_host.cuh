@@ -6,6 +6,7 @@
 #include <stdint.h>
 #include <stdio.h>
 #include <algorithm>
+#include <cstdlib>
 #include <cmath>
 #include <string>
 #include <vector>
@@ -624,10 +625,14 @@ struct Ctx {
     p.nI = (int)nI; p.nPp = (int)nPp; p.NPp = (int)NPp; p.accumulate = accumulate;
     const int grid = std::min(list->n, h->sms);
     if (((i64)(list->n + grid - 1) / grid) * nI >= ((i64)1 << 31)) { status = THC_ERR_OVERFLOW; return; }
-    // Long launches (>= 32 items per CTA) run gated: a cooperative launch (all CTAs co-resident) in which the CTAs wait
-    // for one another every ~2048 grid points of work, so that the L2-ordered work list keeps paying (thc_triple.cuh).
+    // Long launches (>= 64 items per CTA) run gated: a cooperative launch (all CTAs co-resident) in which the CTAs wait
+    // for one another every ~16384 grid points of work, so that the L2-ordered work list keeps paying (thc_triple.cuh).
     p.gate = reinterpret_cast<unsigned int*>(list->dev + list->n);
-    p.gate_every = (h->tp_gate && list->n >= 32 * grid) ? (int)std::max<i64>(1, std::min<i64>(32, 2048 / std::max<i64>(1, nI))) : 0;
+    // Period: 16384 grid points of work, at most 32 items (measured at config 3, step time by period in grid points: none
+    // 36.12 s at the power cap, 512 35.29, 2048 34.98, 4096 34.52, 8192 34.27, 16384 34.17: every barrier costs the wait for
+    // the slowest CTA, so as rare as keeps the GPU under its power cap).  Short items (nI < 256, config 4) run ungated: a
+    // barrier every 16 items of 128 points cost 2.3 % there and the launch is not power-limited.
+    p.gate_every = (h->tp_gate && list->n >= 64 * grid && nI >= 256) ? (int)std::max<i64>(1, std::min<i64>(32, 16384 / nI)) : 0;
     prof_start(1, "triple_product", 5.0 * nI * nPp * (double)NPp * NPp);
     if (p.gate_every) {
       check(cudaMemsetAsync(p.gate, 0, sizeof(unsigned int), h->stream));

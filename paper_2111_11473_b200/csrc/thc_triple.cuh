@@ -25,7 +25,7 @@
 //     chunk (transposed reads of G: rows r, chunks q) -- both read patterns hit eight different chunks;
 //   * work items (p-tile, q-tile, r-tile) come from a host-built list ordered in groups of 8 p-tiles x 6 q-tiles x 3
 //     r-tiles, so that the ~148 CTAs running at the same time share their operand tiles in L2.  That only works while
-//     they run in step: long launches are cooperative and the CTAs wait for one another every ~2048 grid points of work
+//     they run in step: long launches are cooperative and the CTAs wait for one another every ~16384 grid points of work
 //     (TripleParams::gate); ungated they drift apart and two tiles out of three come from DRAM (2.9 TB/s, +100 W).
 #pragma once
 #include <cuda.h>
