@@ -34,6 +34,9 @@
  *     error (if any) is kept in the handle: thc_last_error.
  *   - Pointers must be 8-byte aligned; 16-byte alignment (and even o, v, NP, NX) selects the vectorised
  *     load path, anything else the scalar one.  There is no CPU fallback of any kind.
+ *   - The long launches of Alg.6 line 11 are cooperative launches (one CTA per SM, the CTAs wait for one another at
+ *     intervals so that they share operand tiles in L2): they start once every SM is free, so work of other streams
+ *     that occupies SMs delays them.
  */
 #ifndef THC_H_
 #define THC_H_
